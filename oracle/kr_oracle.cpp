@@ -481,13 +481,21 @@ int32_t step_cell(const kr_oracle_network& n, double rho, double& T_io, double* 
     return st | ST_FAILED_REVERTED;                      // T_io, y_io untouched
   }
 
-  // step 9: finalise (PAPER.md:212-216 stages 1-2)
+  // step 9: finalise (PAPER.md:212-216 stages 1-2).  Stage 1: negatives -> 0.  Stage 2 "corrects the
+  // violation in element abundances brought by step 1": the amount stage 1 added to row nu,
+  // -sum_s N_{nu,s} min(y_s, 0), is taken back from that row's reservoir species (reading R12: equal to the
+  // paper's initial-minus-final element totals up to the solver's own conservation error, which is rounding;
+  // forming it from the clamped amounts keeps a trace reservoir from absorbing eps * total).
   if (o.finalize) {
+    std::vector<Real> removed(E, Real(0));
+    bool any = false;
     for (int s = 0; s < S; ++s)
-      if (w.un[s] < Real(0)) { w.un[s] = Real(0); st |= ST_CLAMPED_NEG; }
-    for (int nu = 0; nu < E; ++nu) {
-      Real delta = Real(0);
-      for (int s = 0; s < S; ++s) delta += Real(n.comp[size_t(nu) * S + s]) * (w.uin[s] - w.un[s]);
+      if (w.un[s] < Real(0)) {
+        for (int nu = 0; nu < E; ++nu) removed[nu] += Real(n.comp[size_t(nu) * S + s]) * w.un[s];
+        w.un[s] = Real(0); st |= ST_CLAMPED_NEG; any = true;
+      }
+    for (int nu = 0; any && nu < E; ++nu) {
+      if (removed[nu] == Real(0)) continue;
       int res = -1, second = -1;
       for (int s = 0; s < S; ++s) {
         if (!n.reservoir_candidates[size_t(nu) * S + s]) continue;
@@ -496,7 +504,7 @@ int32_t step_cell(const kr_oracle_network& n, double rho, double& T_io, double* 
       }
       if (res < 0) { st |= ST_NO_RESERVOIR; continue; }
       if (second >= 0) margin_update(margin, double(w.un[res]), double(w.un[second]));
-      w.un[res] = w.un[res] + delta / Real(n.comp[size_t(nu) * S + res]);
+      w.un[res] = w.un[res] + removed[nu] / Real(n.comp[size_t(nu) * S + res]);
       if (w.un[res] < Real(0)) st |= ST_NEEDS_STAGE3;
     }
   }
