@@ -1,0 +1,169 @@
+/* kratos_chem.h -- C ABI of the B200-native per-cell implicit thermochemistry step.
+ *
+ * What the library computes (arxiv 2504.04941, "PAPER.md"):
+ *   the per-cell ODE system  dn^i/dt = sum A^i_jk n^j n^k + sum B^i_j n^j,  d(eps)/dt = Gamma - Lambda
+ *   (eq. 15) with modified-Arrhenius two-body rates (eq. 16),
+ *   per-cell unary (photo / cosmic-ray) rates (eq. 17), the analytic Jacobian of
+ *   abundances plus temperature (eqs. 18-20), integrated by an implicit
+ *   ("semi-implicit") scheme with adaptive sub-steps, each
+ *   Newton iteration solving one small dense system by LU with implicit-scaled row pivoting
+ *   (Algorithm 1), followed by the post-processing repair stages 1-2 and the
+ *   retry / revert policy.  Readings of everything the paper leaves open are
+ *   listed in DESIGN.md ("Readings R1-R22").
+ *
+ * Conventions
+ *   - All functions return int: KR_OK (0) or a negative KR_E* code; kr_last_error() gives a
+ *     thread-local message for the last failing call on the calling thread.
+ *   - "host" / "device" is stated for every pointer.  The library never frees or reallocates a
+ *     caller buffer.  It owns its network tables and a small device workspace (work counter,
+ *     statistics), created in kr_network_create and released in kr_network_destroy.
+ *   - State variable: y_s = n_s m_u / rho (dimensionless; R10), cell-major y[n_cells*S].
+ *   - CGS units: rho g cm^-3, T K, dt s, A cm^3 s^-1 (two-body) or s^-1 (unary), Ea_over_k K,
+ *     q_ext erg.
+ *   - Every step of the path runs in CUDA kernels for sm_100a.  There is no CPU fallback: without a
+ *     CUDA device every compute call fails with KR_ECUDA.
+ */
+#ifndef KRATOS_CHEM_H
+#define KRATOS_CHEM_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { KR_OK = 0, KR_EINVAL = -1, KR_ENETWORK = -2, KR_ECUDA = -3, KR_EUNSUPPORTED = -4 };
+
+/* reaction flag bits (kr_network_desc.flags) */
+enum { KR_F_REVERSIBLE = 1,   /* reverse rate from detailed balance, k_r = k_f / K_c(T) (R5) */
+       KR_F_THIRD_BODY = 2,   /* both directions multiplied by M = sum_s eff_s n_s (R6)      */
+       KR_F_CONST_UNARY = 4,  /* k = A, no temperature dependence (cosmic ray; R17)          */
+       KR_F_AUX_UNARY = 8 };  /* k = A * aux[aux_index][cell] (photo rate, eq. 17; R16)      */
+
+/* per-cell status bits (status[] of kr_thermochem_step_ex) */
+enum { KR_ST_REJECTED_ONCE = 1,    /* at least one sub-step was rejected and retried */
+       KR_ST_CLAMPED_NEG = 2,      /* post-processing stage 1 zeroed a negative abundance */
+       KR_ST_FAILED_REVERTED = 8,  /* controller gave up; the cell's T and y are left as given (R13) */
+       KR_ST_T_CLAMPED = 16,       /* input T was outside [T_lo, T_hi] and was clamped */
+       KR_ST_NO_RESERVOIR = 32,    /* stage 2: a conservation row has no single-element species */
+       KR_ST_NEEDS_STAGE3 = 64 };  /* stage 2 drove the reservoir negative (stage 3 is not built) */
+
+/* precision_mode */
+enum { KR_FP64 = 0,    /* everything in fp64 */
+       KR_MIXED = 1 }; /* fp32 Jacobian/LU on the scaled system, fp64 residual, refinement (R15) */
+
+/* per-cell mapping (kr_network_set_mapping); KR_MAP_AUTO picks from N by measurement */
+enum { KR_MAP_AUTO = 0, KR_MAP_THREAD = 1, KR_MAP_WARP = 2, KR_MAP_CTA = 3 };
+
+typedef struct kr_network kr_network; /* opaque; owns host + device tables and the workspace */
+
+/* Network description.  All pointers are HOST pointers, read during kr_network_create only. */
+typedef struct {
+  int32_t n_elem, n_species, n_reac; /* E conservation rows (elements, optional charge row), S, R */
+  const double *elem_mass;           /* [E] amu (0 on a charge row) */
+  const int32_t *composition;        /* [E*S] row-major N_{nu,s}; signed on a charge row */
+  const int32_t *reac_idx, *reac_nu; /* [R*3] reactant species index (-1 = unused) and coefficient >= 1 */
+  const int32_t *prod_idx, *prod_nu; /* [R*3] products, same packing; a species appears once per side */
+  const double *A, *beta, *Ea_over_k; /* [R] k_f = A (T/300K)^beta exp(-Ea_over_k/T) (eq. 16, R4) */
+  const int32_t *flags;              /* [R] KR_F_* bits */
+  const int32_t *aux_index;          /* [R] row of aux[] for KR_F_AUX_UNARY reactions, else -1; may be NULL */
+  const double *tb_eff;              /* [R*S] third-body efficiencies, or NULL (all 1) */
+  const double *q_ext;               /* [R] erg deposited per forward event, or NULL (0) */
+  const double *nasa_lo, *nasa_hi;   /* [S*7] a1..a7 for T <= T_mid[s] / T > T_mid[s] (R7) */
+  const double *T_mid;               /* [S] */
+  double T_lo, T_hi;                 /* clamp / validity range (R19) */
+  int32_t energy_equation;           /* 0: isothermal, N = S;  1: T is an unknown, N = S + 1 (eq. 18) */
+} kr_network_desc;
+
+/* Solver options; kr_default_opts() fills the defaults of DESIGN.md "Algorithm" (h0_mode = 1). */
+typedef struct {
+  int32_t max_newton;   /* K: Newton iterations per sub-step (>= 1) */
+  int32_t fixed_newton; /* 1: always K iterations (parity runs); 0: stop at the first e_k <= 1, bail out on divergence */
+  int32_t h0_mode;      /* 0: first sub-step h = dt; 1: h = min(dt, eta / max_s |ydot_s|/(|y_s|+y_floor)) */
+  double rtol, atol_y, atol_T; /* Newton convergence: e = max_i |delta_i| / (rtol |u_i| + atol_i) <= 1 */
+  double neg_tol;       /* reject a sub-step whose smallest abundance is < -neg_tol */
+  double eta, y_floor;  /* first-sub-step rule (h0_mode 1) */
+  double shrink;        /* h <- h * shrink after a rejection (0 < shrink < 1) */
+  double grow_fast, grow_mid; /* h <- h * grow_fast if it <= it_fast, * grow_mid if it <= it_mid */
+  double chg_floor, chg_max;  /* optional accuracy limiter; off when chg_max = +inf */
+  int32_t it_fast, it_mid, max_substeps;
+  int32_t finalize;     /* 1: run post-processing stages 1-2; 0: skip */
+  double h_min_rel;     /* fail when h < h_min_rel * (first sub-step size) */
+  double bail_ratio;    /* early-exit mode: abort the sub-step when e_k > bail_ratio * e_{k-1}, k >= 2 */
+} kr_solver_opts;
+
+/* Work counters of one call, summed over cells. */
+typedef struct {
+  int64_t n_substeps; /* accepted sub-steps */
+  int64_t n_rejected; /* rejected sub-steps */
+  int64_t n_newton;   /* Newton iterations = Jacobian assemblies */
+  int64_t n_lu;       /* LU factorisations (+ substitutions) */
+  int64_t n_rate_evals; /* evaluations of the rate-constant set (thermo + Arrhenius + K_c) */
+  int64_t n_failed;   /* cells reverted */
+} kr_step_stats;
+
+/* Build a network.  desc and everything it points to are host memory, copied; the call validates
+ * indices, reaction order <= 3 per side (R20) and element conservation N . dnu_r = 0 of every
+ * reaction against the composition matrix -> KR_ENETWORK when violated, builds
+ * the device tables (reaction records, Jacobian gather lists) and picks the per-cell mapping.
+ * Needs a CUDA device (current device of the calling thread) -> KR_ECUDA without one. */
+int kr_network_create(const kr_network_desc *desc, kr_network **out);
+void kr_network_destroy(kr_network *net);
+
+void kr_default_opts(kr_solver_opts *opts);                      /* host pointer, filled */
+int kr_network_set_options(kr_network *net, const kr_solver_opts *opts); /* host pointer, copied; KR_EINVAL on nonsense */
+int kr_network_get_options(const kr_network *net, kr_solver_opts *opts);
+/* Stream used by kr_thermochem_step (a cudaStream_t passed as void*; NULL = legacy default stream). */
+int kr_set_stream(kr_network *net, void *cuda_stream);
+/* Override the mapping picked from N: mapping = KR_MAP_*, threads_per_cell = 0 (auto) or a multiple
+ * of 32 for KR_MAP_WARP (32) / KR_MAP_CTA (64..256).  KR_EUNSUPPORTED when N does not fit it. */
+int kr_network_set_mapping(kr_network *net, int32_t mapping, int32_t threads_per_cell);
+/* Query: N (unknowns per cell), mapping in use, threads per cell, dynamic shared memory per block. */
+int kr_network_info(const kr_network *net, int32_t *n_unknowns, int32_t *mapping, int32_t *threads_per_cell,
+                    int32_t *smem_bytes);
+
+/* One implicit chemistry step of size dt for n_cells independent cells (DESIGN.md steps 1-9).
+ *   rho  [n_cells]    DEVICE, read-only (fixed during the step)
+ *   T    [n_cells]    DEVICE, in/out when the energy equation is on, read-only otherwise
+ *   y    [n_cells*S]  DEVICE, cell-major, in/out
+ *   precision_mode    KR_FP64 or KR_MIXED, anything else -> KR_EINVAL
+ * Runs asynchronously on the stream set by kr_set_stream; returns after the launches are queued.
+ * A cell whose controller fails is left untouched (reverted); that is not a call failure.
+ * A network with KR_F_AUX_UNARY reactions needs kr_thermochem_step_ex (KR_EINVAL here). */
+int kr_thermochem_step(kr_network *net, int64_t n_cells, const double *rho, double *T, double *y, double dt,
+                       int precision_mode);
+
+/* Same, plus per-cell auxiliary rates, status and statistics.
+ *   aux    [n_aux*n_cells] DEVICE, row a = values of auxiliary field a (photo rate, shielding), or NULL
+ *   status [n_cells]       DEVICE int32, KR_ST_* bits per cell, or NULL
+ *   stats                  HOST, or NULL; non-NULL forces one stream synchronisation before returning
+ *   cuda_stream            stream for this call (void* cudaStream_t; NULL = the stream of kr_set_stream) */
+int kr_thermochem_step_ex(kr_network *net, int64_t n_cells, const double *rho, double *T, double *y, double dt,
+                          int precision_mode, const double *aux, int32_t n_aux, int32_t *status,
+                          kr_step_stats *stats, void *cuda_stream);
+
+/* Host-buffer convenience used for the end-to-end measurement: same arguments as kr_thermochem_step_ex
+ * but rho, T, y, aux, status are HOST pointers; the call stages them through device buffers cached on
+ * the handle (host->device copies, the step, device->host copies of T, y, status) and synchronises. */
+int kr_thermochem_step_host(kr_network *net, int64_t n_cells, const double *rho, double *T, double *y, double dt,
+                            int precision_mode, const double *aux, int32_t n_aux, int32_t *status,
+                            kr_step_stats *stats);
+
+/* Number of kernel launches the last step call on this handle queued (for bench.py's gpu_launches). */
+int kr_last_launch_count(const kr_network *net);
+
+/* Layout boundary on its own (DESIGN.md a1/a9): cell-major y[n_cells*S] <-> species-SoA ys[S][n_cells],
+ * DEVICE pointers, coalesced both ways through shared-memory tiles.  Exposed for hydro codes that keep
+ * species-SoA fields; kr_thermochem_step does its own transposition inside the solve kernels. */
+int kr_layout_cell_to_soa(const double *y_cell, double *y_soa, int64_t n_cells, int32_t S, void *cuda_stream);
+int kr_layout_soa_to_cell(const double *y_soa, double *y_cell, int64_t n_cells, int32_t S, void *cuda_stream);
+
+/* FP64 FMA peak microbenchmark (independent DFMA chains on every SM).  Returns
+ * the achieved TFLOP/s in *tflops (host) measured with CUDA events over n_iter inner iterations. */
+int kr_measure_fp64_peak(int32_t n_iter, double *tflops);
+
+const char *kr_last_error(void);
+const char *kr_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* KRATOS_CHEM_H */

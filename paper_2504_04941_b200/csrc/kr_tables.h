@@ -1,0 +1,75 @@
+// kr_tables.h -- plain-data views of a network and of the solver options as the kernels see them.
+// Internal to the CUDA path (never included by oracle/).  All pointers are DEVICE pointers.
+#pragma once
+
+// physical constants, CGS
+#define KR_K_B 1.380649e-16
+#define KR_M_U 1.66053906660e-24
+#define KR_P0 1.01325e6
+#define KR_T_REF 300.0
+#define KR_EXP_CLAMP 690.0
+
+struct KrNetDev {
+  int E, S, R, N;        // conservation rows, species, reactions, unknowns (S or S+1)
+  int energy;            // 1: T is the last unknown
+  int n_aux;             // aux rows the network needs
+  int any_rev;           // some reaction is reversible (thermo needed for K_c)
+  int any_tb, any_qext;  // third-body / external heat present
+  int ld;                // leading dimension of the per-cell matrix in the group kernels (odd, >= N+1)
+  double T_lo, T_hi;
+  double ln_p0_kB;       // ln(p0 / k_B)
+  // reaction records
+  const int* sp;         // [R*6] species of slot k: 0..2 reactants, 3..5 products, -1 = unused
+  const int* nu;         // [R*6] stoichiometric coefficient of the slot (0 when unused)
+  const int* flags;      // [R]
+  const int* auxi;       // [R]
+  const int* dnu_tot;    // [R] sum products nu - sum reactants nu
+  const double* c0;      // [R] ln A - beta ln T_ref
+  const double* A;       // [R]
+  const double* beta;    // [R]
+  const double* Ea;      // [R]
+  const double* qk;      // [R] q_ext / k_B
+  const double* tb_eff;  // [R*S] (valid when any_tb)
+  // thermo
+  const double* nasa;    // [S*14]: 7 low-range then 7 high-range coefficients
+  const double* T_mid;   // [S]
+  // conservation rows
+  const int* comp;       // [E*S]
+  const int* resv;       // [E*S] 1 where species s is a reservoir candidate of row nu
+  // gather lists of the group (warp / CTA per cell) kernels
+  const int* row_ptr;    // [S+1]  row list of species s: entries row_ptr[s]..row_ptr[s+1]
+  const int* row_ent;    // packed (reaction << 8) | (dnu + 128)
+  const int* col_ptr;    // [S+1]  column list of species m
+  const int* col_ent;    // packed (reaction << 4) | slot, slot 0..5 = participant slot, 15 = third-body only
+};
+
+struct KrOptsDev {
+  int max_newton, fixed_newton, h0_mode, it_fast, it_mid, max_substeps, finalize;
+  double rtol, atol_y, atol_T, neg_tol, eta, y_floor, shrink, grow_fast, grow_mid, chg_floor, chg_max;
+  double h_min_rel, bail_ratio;
+};
+
+struct KrStepArgs {
+  long long n_cells;
+  const double* rho;
+  double* T;
+  double* y;
+  const double* aux;
+  int* status;
+  double dt;
+  unsigned long long* counter;   // work queue head
+  unsigned long long* stats;     // [6] device counters
+};
+
+// status bits (mirror of include/kratos_chem.h, kept numeric so that device code needs no host header)
+#define KR_DST_REJECTED 1
+#define KR_DST_CLAMPED_NEG 2
+#define KR_DST_FAILED 8
+#define KR_DST_T_CLAMPED 16
+#define KR_DST_NO_RESERVOIR 32
+#define KR_DST_NEEDS_STAGE3 64
+
+#define KR_DF_REV 1
+#define KR_DF_TB 2
+#define KR_DF_CONST 4
+#define KR_DF_AUX 8
