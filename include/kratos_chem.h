@@ -51,7 +51,11 @@ enum { KR_FP64 = 0,    /* everything in fp64 */
        KR_MIXED = 1 }; /* fp32 Jacobian/LU on the scaled system, fp64 residual, refinement (R15) */
 
 /* per-cell mapping (kr_network_set_mapping); KR_MAP_AUTO picks from N by measurement */
-enum { KR_MAP_AUTO = 0, KR_MAP_THREAD = 1, KR_MAP_WARP = 2, KR_MAP_CTA = 3 };
+enum { KR_MAP_AUTO = 0,
+       KR_MAP_THREAD = 1,        /* one lane per cell; kernel SPECIALISED to the network at create time (NVRTC) */
+       KR_MAP_WARP = 2,          /* one warp per cell, table driven */
+       KR_MAP_CTA = 3,           /* 64..256 threads per cell, table driven */
+       KR_MAP_THREAD_TABLE = 4 };/* one lane per cell, table driven (no run-time compilation) */
 
 typedef struct kr_network kr_network; /* opaque; owns host + device tables and the workspace */
 
@@ -147,6 +151,17 @@ int kr_thermochem_step_host(kr_network *net, int64_t n_cells, const double *rho,
                             int precision_mode, const double *aux, int32_t n_aux, int32_t *status,
                             kr_step_stats *stats);
 
+/* One-line description of the kernel the current mapping launches (registers, blocks per SM ...), host buffer. */
+int kr_network_kernel_desc(const kr_network *net, char *buf, int64_t cap);
+/* The generated translation unit (struct KrNet of constexpr tables) the specialised kernel is compiled against;
+ * host only, needs no GPU.  Returns the length, or a negative KR_E* code; buf may be NULL to query the length. */
+int kr_network_spec_source(const kr_network_desc *desc, char *buf, int64_t cap);
+
+/* Compile (NVRTC, sm_100a; needs no GPU) the specialised kernel of a network without loading it: the build-time
+ * check of the run-time compiled path.  *cubin_bytes (host) receives the cubin size, log (host, may be NULL) the
+ * compiler log.  KR_ECUDA when NVRTC is unavailable or the compilation fails. */
+int kr_network_spec_compile(const kr_network_desc *desc, int64_t *cubin_bytes, char *log, int64_t log_cap);
+
 /* Number of kernel launches the last step call on this handle queued (for bench.py's gpu_launches). */
 int kr_last_launch_count(const kr_network *net);
 
@@ -155,6 +170,10 @@ int kr_last_launch_count(const kr_network *net);
  * species-SoA fields; kr_thermochem_step does its own transposition inside the solve kernels. */
 int kr_layout_cell_to_soa(const double *y_cell, double *y_soa, int64_t n_cells, int32_t S, void *cuda_stream);
 int kr_layout_soa_to_cell(const double *y_soa, double *y_cell, int64_t n_cells, int32_t S, void *cuda_stream);
+
+/* Accuracy probe of the two lean FP64 primitives the specialised kernels use instead of the library divide and exp
+ * (csrc/kr_math.cuh): rcp[i] = 1/x[i] (x normal), ex[i] = exp(min(x[i], 690)).  DEVICE pointers, n elements. */
+int kr_math_probe(const double *x, double *rcp, double *ex, int64_t n, void *cuda_stream);
 
 /* FP64 FMA peak microbenchmark (independent DFMA chains on every SM).  Returns
  * the achieved TFLOP/s in *tflops (host) measured with CUDA events over n_iter inner iterations. */

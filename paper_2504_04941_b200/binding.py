@@ -19,14 +19,14 @@ LIB_PATH = os.path.join(_HERE, "libkratos_chem.so")
 
 KR_OK, KR_EINVAL, KR_ENETWORK, KR_ECUDA, KR_EUNSUPPORTED = 0, -1, -2, -3, -4
 KR_FP64, KR_MIXED = 0, 1
-KR_MAP_AUTO, KR_MAP_THREAD, KR_MAP_WARP, KR_MAP_CTA = 0, 1, 2, 3
+KR_MAP_AUTO, KR_MAP_THREAD, KR_MAP_WARP, KR_MAP_CTA, KR_MAP_THREAD_TABLE = 0, 1, 2, 3, 4
 ST_REJECTED_ONCE, ST_CLAMPED_NEG, ST_FAILED_REVERTED, ST_T_CLAMPED, ST_NO_RESERVOIR, ST_NEEDS_STAGE3 = 1, 2, 8, 16, 32, 64
 
 EXPORTS = [
     "kr_network_create", "kr_network_destroy", "kr_default_opts", "kr_network_set_options",
     "kr_network_get_options", "kr_set_stream", "kr_network_set_mapping", "kr_network_info",
-    "kr_thermochem_step", "kr_thermochem_step_ex", "kr_thermochem_step_host", "kr_last_launch_count",
-    "kr_layout_cell_to_soa", "kr_layout_soa_to_cell", "kr_measure_fp64_peak", "kr_last_error", "kr_version",
+    "kr_network_kernel_desc", "kr_network_spec_source", "kr_network_spec_compile", "kr_thermochem_step", "kr_thermochem_step_ex", "kr_thermochem_step_host", "kr_last_launch_count",
+    "kr_layout_cell_to_soa", "kr_layout_soa_to_cell", "kr_math_probe", "kr_measure_fp64_peak", "kr_last_error", "kr_version",
 ]
 
 _dp = C.POINTER(C.c_double)
@@ -95,9 +95,13 @@ def load() -> C.CDLL:
     lib.kr_thermochem_step_host.argtypes = [vp, C.c_int64, vp, vp, vp, C.c_double, C.c_int, vp, C.c_int32, vp,
                                             C.POINTER(StepStats)]
     lib.kr_last_launch_count.argtypes = [vp]
+    lib.kr_network_kernel_desc.argtypes = [vp, C.c_char_p, C.c_int64]
+    lib.kr_network_spec_source.argtypes = [C.POINTER(NetworkDesc), C.c_char_p, C.c_int64]
+    lib.kr_network_spec_compile.argtypes = [C.POINTER(NetworkDesc), C.POINTER(C.c_int64), C.c_char_p, C.c_int64]
     lib.kr_layout_cell_to_soa.argtypes = [vp, vp, C.c_int64, C.c_int32, vp]
     lib.kr_layout_soa_to_cell.argtypes = [vp, vp, C.c_int64, C.c_int32, vp]
     lib.kr_measure_fp64_peak.argtypes = [C.c_int32, _dp]
+    lib.kr_math_probe.argtypes = [vp, vp, vp, C.c_int64, vp]
     lib.kr_last_error.restype = C.c_char_p
     lib.kr_version.restype = C.c_char_p
     _lib = lib
@@ -153,6 +157,42 @@ def measure_fp64_peak(n_iter: int = 4096) -> float:
     v = C.c_double()
     _check(load().kr_measure_fp64_peak(int(n_iter), C.byref(v)))
     return v.value
+
+
+def make_desc(net):
+    """(kr_network_desc, keep-alive dict) from a ``workloads.Network``-shaped object."""
+    k = dict(
+        elem_mass=_f64(net.elem_mass), composition=_i32(net.composition),
+        reac_idx=_i32(net.reac_idx), reac_nu=_i32(net.reac_nu), prod_idx=_i32(net.prod_idx),
+        prod_nu=_i32(net.prod_nu), A=_f64(net.A), beta=_f64(net.beta), Ea=_f64(net.Ea_over_k),
+        flags=_i32(net.flags), aux_index=_i32(net.aux_index), tb_eff=_f64(net.tb_eff), q_ext=_f64(net.q_ext),
+        nasa_lo=_f64(net.nasa_lo), nasa_hi=_f64(net.nasa_hi), T_mid=_f64(net.T_mid))
+    d = NetworkDesc(net.n_elem, net.n_species, net.n_reac, _d(k["elem_mass"]), _i(k["composition"]),
+                    _i(k["reac_idx"]), _i(k["reac_nu"]), _i(k["prod_idx"]), _i(k["prod_nu"]),
+                    _d(k["A"]), _d(k["beta"]), _d(k["Ea"]), _i(k["flags"]), _i(k["aux_index"]),
+                    _d(k["tb_eff"]), _d(k["q_ext"]), _d(k["nasa_lo"]), _d(k["nasa_hi"]), _d(k["T_mid"]),
+                    float(net.T_lo), float(net.T_hi), int(net.energy_equation))
+    return d, k
+
+
+def spec_source(net) -> str:
+    """kr_network_spec_source: the generated constexpr-table translation unit (host only)."""
+    d, keep = make_desc(net)
+    n = load().kr_network_spec_source(C.byref(d), None, 0)
+    if n < 0:
+        _check(n)
+    buf = C.create_string_buffer(n + 1)
+    load().kr_network_spec_source(C.byref(d), buf, n + 1)
+    return buf.value.decode()
+
+
+def spec_compile(net) -> dict:
+    """kr_network_spec_compile: NVRTC-compile the specialised kernel for sm_100a (no GPU needed)."""
+    d, keep = make_desc(net)
+    size = C.c_int64()
+    log = C.create_string_buffer(1 << 16)
+    _check(load().kr_network_spec_compile(C.byref(d), C.byref(size), log, 1 << 16))
+    return {"cubin_bytes": size.value, "log": log.value.decode()}
 
 
 class Network:
@@ -215,6 +255,11 @@ class Network:
         _check(load().kr_network_info(self._h, C.byref(a), C.byref(b), C.byref(c), C.byref(d)))
         return {"n_unknowns": a.value, "mapping": b.value, "threads_per_cell": c.value, "smem_bytes": d.value}
 
+    def kernel_desc(self) -> str:
+        buf = C.create_string_buffer(512)
+        _check(load().kr_network_kernel_desc(self._h, buf, 512))
+        return buf.value.decode()
+
     def last_launch_count(self) -> int:
         return int(load().kr_last_launch_count(self._h))
 
@@ -243,6 +288,10 @@ class Network:
                                               int(precision_mode), _ptr(aux), n_aux, _ptr(status),
                                               C.byref(st) if want_stats else None))
         return st.as_dict() if want_stats else None
+
+
+def math_probe(x, rcp, ex, n: int, stream: int = 0) -> None:
+    _check(load().kr_math_probe(_ptr(x), _ptr(rcp), _ptr(ex), int(n), C.c_void_p(stream or None)))
 
 
 def layout_cell_to_soa(y_cell, y_soa, n_cells: int, S: int, stream: int = 0) -> None:

@@ -6,7 +6,7 @@ smallest relative margin of any controller decision.  A cell is *comparable* whe
   (beta)  every accept/reject/early-exit/growth decision had a margin > 1e-6 (a last-bit difference
           cannot flip it), and neither run reverted the cell.
   (gamma) the oracle's own double result moves by < 1e-10 when its inputs are perturbed by 1e-13 relative
-          (two seeded perturbations): a Newton iteration started far from the solution (config 0 takes
+          (four seeded perturbations of y, T, rho): a Newton iteration started far from the solution (config 0 takes
           h = dt first) can amplify rounding differences by many decades BEFORE a decision is taken, which
           (alpha) and (beta) alone do not see.
 On comparable cells the CUDA result must equal the oracle's within 1e-9 relative on every abundance
@@ -37,11 +37,12 @@ def oracle_reference(oracle_mod, net, cells, opts, n_threads=8):
     if net.energy_equation:
         alpha = np.maximum(alpha, np.abs(T - Tw) / np.abs(Tw))
     gamma = np.zeros_like(alpha)
-    for k in range(2):
+    for k in range(4):
         rng = np.random.default_rng(777 + k)
         pc = cells.copy()
         pc.y = cells.y * (1.0 + 1e-13 * rng.choice([-1.0, 1.0], size=cells.y.shape))
-        pc.T = cells.T * (1.0 + 1e-14 * rng.choice([-1.0, 1.0], size=cells.T.shape))
+        pc.T = cells.T * (1.0 + (1e-14 if k < 2 else 1e-13) * rng.choice([-1.0, 1.0], size=cells.T.shape))
+        pc.rho = cells.rho * (1.0 + 1e-13 * rng.choice([-1.0, 1.0], size=cells.rho.shape))
         Tp, yp, stp, _, mp = on.step(pc, n_threads=n_threads, want_margins=True)
         g = rel_err(yp, y).max(axis=1)
         if net.energy_equation:

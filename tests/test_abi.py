@@ -77,6 +77,17 @@ def test_validation_runs_on_the_host_before_any_device_work(B):
         assert e.value.code == B.KR_ECUDA and "no CPU path" in str(e.value)
 
 
+@pytest.mark.parametrize("idx", [0, 1, 2])
+def test_specialised_kernel_compiles_for_sm100a_without_a_gpu(B, idx):
+    """The run-time compiled path (NVRTC) is checked at build time: source generation + compilation need no GPU."""
+    net = w.make_network(idx)
+    src = B.spec_source(net)
+    assert "struct KrNet" in src and f"S = {net.n_species}" in src and f"R = {net.n_reac}" in src
+    out = B.spec_compile(net)
+    assert out["cubin_bytes"] > 10000
+    assert "error" not in out["log"].lower()
+
+
 def test_null_and_nonsense_arguments(B):
     lib = B.load()
     assert lib.kr_network_create(None, None) == B.KR_EINVAL
