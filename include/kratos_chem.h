@@ -41,6 +41,7 @@ enum { KR_F_REVERSIBLE = 1,   /* reverse rate from detailed balance, k_r = k_f /
 /* per-cell status bits (status[] of kr_thermochem_step_ex) */
 enum { KR_ST_REJECTED_ONCE = 1,    /* at least one sub-step was rejected and retried */
        KR_ST_CLAMPED_NEG = 2,      /* post-processing stage 1 zeroed a negative abundance */
+       KR_ST_FP64_FALLBACK = 4,    /* mixed precision: fp32 could not resolve a linear system of this cell; it was redone in fp64 */
        KR_ST_FAILED_REVERTED = 8,  /* controller gave up; the cell's T and y are left as given (R13) */
        KR_ST_T_CLAMPED = 16,       /* input T was outside [T_lo, T_hi] and was clamped */
        KR_ST_NO_RESERVOIR = 32,    /* stage 2: a conservation row has no single-element species */
@@ -48,14 +49,16 @@ enum { KR_ST_REJECTED_ONCE = 1,    /* at least one sub-step was rejected and ret
 
 /* precision_mode */
 enum { KR_FP64 = 0,    /* everything in fp64 */
-       KR_MIXED = 1 }; /* fp32 Jacobian/LU on the scaled system, fp64 residual, refinement (R15) */
+       KR_MIXED = 1 }; /* fp32 Jacobian + elimination on the row-scaled system, fp64 residuals, iterative refinement (R15); a cell
+                        * whose refinement does not contract is redone in fp64 (two launches).  Built for N <= 64. */
 
 /* per-cell mapping (kr_network_set_mapping); KR_MAP_AUTO picks from N by measurement */
 enum { KR_MAP_AUTO = 0,
        KR_MAP_THREAD = 1,        /* one lane per cell; kernel SPECIALISED to the network at create time (NVRTC) */
-       KR_MAP_WARP = 2,          /* one warp per cell, table driven */
-       KR_MAP_CTA = 3,           /* 64..256 threads per cell, table driven */
-       KR_MAP_THREAD_TABLE = 4 };/* one lane per cell, table driven (no run-time compilation) */
+       KR_MAP_WARP = 2,          /* one warp per cell: matrix in register tiles, kernel compiled for the network's sizes (NVRTC) */
+       KR_MAP_CTA = 3,           /* 64..256 threads per cell: register tiles on 64 threads (N <= 64), else matrix in shared memory */
+       KR_MAP_THREAD_TABLE = 4,  /* one lane per cell, table driven (no run-time compilation) */
+       KR_MAP_GROUP_TABLE = 5 }; /* 32..256 threads per cell, matrix in shared memory, table driven (no run-time compilation) */
 
 typedef struct kr_network kr_network; /* opaque; owns host + device tables and the workspace */
 
@@ -161,6 +164,17 @@ int kr_network_spec_source(const kr_network_desc *desc, char *buf, int64_t cap);
  * check of the run-time compiled path.  *cubin_bytes (host) receives the cubin size, log (host, may be NULL) the
  * compiler log.  KR_ECUDA when NVRTC is unavailable or the compilation fails. */
 int kr_network_spec_compile(const kr_network_desc *desc, int64_t *cubin_bytes, char *log, int64_t log_cap);
+
+/* Build-time check of the register-tile kernel (csrc/kr_wpc.cuh) for a network: compile it with NVRTC for sm_100a without
+ * loading it (needs no GPU).  precision_mode KR_FP64 / KR_MIXED, warps_per_cell 1 or 2.  *cubin_bytes (host) receives the
+ * cubin size, log (host, may be NULL) the compiler log, cubin (host, may be NULL) up to cubin_cap bytes of the image. */
+int kr_network_wpc_compile(const kr_network_desc *desc, int precision_mode, int32_t warps_per_cell, int64_t *cubin_bytes,
+                           char *log, int64_t log_cap, void *cubin, int64_t cubin_cap);
+
+/* Mixed precision only, counters of the last step call summed over cells: refinement passes (fp64 residual + fp32
+ * replay), and cells whose fp32 factorisation could not be refined and that were redone by the fp64 kernel (status bit
+ * KR_ST_FP64_FALLBACK).  Synchronises the device.  HOST pointers, either may be NULL. */
+int kr_last_mixed_stats(kr_network *net, int64_t *n_refine, int64_t *n_fp64_cells);
 
 /* Number of kernel launches the last step call on this handle queued (for bench.py's gpu_launches). */
 int kr_last_launch_count(const kr_network *net);

@@ -19,13 +19,13 @@ LIB_PATH = os.path.join(_HERE, "libkratos_chem.so")
 
 KR_OK, KR_EINVAL, KR_ENETWORK, KR_ECUDA, KR_EUNSUPPORTED = 0, -1, -2, -3, -4
 KR_FP64, KR_MIXED = 0, 1
-KR_MAP_AUTO, KR_MAP_THREAD, KR_MAP_WARP, KR_MAP_CTA, KR_MAP_THREAD_TABLE = 0, 1, 2, 3, 4
-ST_REJECTED_ONCE, ST_CLAMPED_NEG, ST_FAILED_REVERTED, ST_T_CLAMPED, ST_NO_RESERVOIR, ST_NEEDS_STAGE3 = 1, 2, 8, 16, 32, 64
+KR_MAP_AUTO, KR_MAP_THREAD, KR_MAP_WARP, KR_MAP_CTA, KR_MAP_THREAD_TABLE, KR_MAP_GROUP_TABLE = 0, 1, 2, 3, 4, 5
+ST_REJECTED_ONCE, ST_CLAMPED_NEG, ST_FP64_FALLBACK, ST_FAILED_REVERTED, ST_T_CLAMPED, ST_NO_RESERVOIR, ST_NEEDS_STAGE3 = 1, 2, 4, 8, 16, 32, 64
 
 EXPORTS = [
     "kr_network_create", "kr_network_destroy", "kr_default_opts", "kr_network_set_options",
     "kr_network_get_options", "kr_set_stream", "kr_network_set_mapping", "kr_network_info",
-    "kr_network_kernel_desc", "kr_network_spec_source", "kr_network_spec_compile", "kr_thermochem_step", "kr_thermochem_step_ex", "kr_thermochem_step_host", "kr_last_launch_count",
+    "kr_network_kernel_desc", "kr_network_spec_source", "kr_network_spec_compile", "kr_network_wpc_compile", "kr_last_mixed_stats", "kr_thermochem_step", "kr_thermochem_step_ex", "kr_thermochem_step_host", "kr_last_launch_count",
     "kr_layout_cell_to_soa", "kr_layout_soa_to_cell", "kr_math_probe", "kr_measure_fp64_peak", "kr_last_error", "kr_version",
 ]
 
@@ -98,6 +98,9 @@ def load() -> C.CDLL:
     lib.kr_network_kernel_desc.argtypes = [vp, C.c_char_p, C.c_int64]
     lib.kr_network_spec_source.argtypes = [C.POINTER(NetworkDesc), C.c_char_p, C.c_int64]
     lib.kr_network_spec_compile.argtypes = [C.POINTER(NetworkDesc), C.POINTER(C.c_int64), C.c_char_p, C.c_int64]
+    lib.kr_network_wpc_compile.argtypes = [C.POINTER(NetworkDesc), C.c_int, C.c_int32, C.POINTER(C.c_int64), C.c_char_p, C.c_int64,
+                                           vp, C.c_int64]
+    lib.kr_last_mixed_stats.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
     lib.kr_layout_cell_to_soa.argtypes = [vp, vp, C.c_int64, C.c_int32, vp]
     lib.kr_layout_soa_to_cell.argtypes = [vp, vp, C.c_int64, C.c_int32, vp]
     lib.kr_measure_fp64_peak.argtypes = [C.c_int32, _dp]
@@ -195,6 +198,21 @@ def spec_compile(net) -> dict:
     return {"cubin_bytes": size.value, "log": log.value.decode()}
 
 
+def wpc_compile(net, precision_mode: int = KR_FP64, warps_per_cell: int = 1, want_cubin: bool = False) -> dict:
+    """kr_network_wpc_compile: NVRTC-compile the register-tile kernel for sm_100a (no GPU needed)."""
+    d, keep = make_desc(net)
+    size = C.c_int64()
+    log = C.create_string_buffer(1 << 16)
+    cap = (8 << 20) if want_cubin else 0
+    img = C.create_string_buffer(cap) if want_cubin else None
+    _check(load().kr_network_wpc_compile(C.byref(d), int(precision_mode), int(warps_per_cell), C.byref(size), log, 1 << 16,
+                                         C.cast(img, C.c_void_p) if want_cubin else None, cap))
+    out = {"cubin_bytes": size.value, "log": log.value.decode()}
+    if want_cubin:
+        out["cubin"] = img.raw[:size.value]
+    return out
+
+
 class Network:
     """kr_network handle built from a ``workloads.Network``-shaped object (kr_network_create)."""
 
@@ -262,6 +280,11 @@ class Network:
 
     def last_launch_count(self) -> int:
         return int(load().kr_last_launch_count(self._h))
+
+    def last_mixed_stats(self) -> dict:
+        a, b = C.c_int64(), C.c_int64()
+        _check(load().kr_last_mixed_stats(self._h, C.byref(a), C.byref(b)))
+        return {"n_refine": int(a.value), "n_fp64_cells": int(b.value)}
 
     # -- the step -----------------------------------------------------------------------------
     def thermochem_step(self, n_cells: int, rho, T, y, dt: float, precision_mode: int = KR_FP64) -> None:

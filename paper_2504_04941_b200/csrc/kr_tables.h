@@ -58,12 +58,18 @@ struct KrStepArgs {
   int* status;
   double dt;
   unsigned long long* counter;   // work queue head
-  unsigned long long* stats;     // [6] device counters
+  unsigned long long* stats;     // [6] device counters (+ [6]: refinement passes of the mixed mode)
+  // mixed precision: cells whose fp32 factorisation cannot be refined are appended to retry_list and redone in fp64
+  long long* retry_list;               // [n_cells] or null
+  unsigned long long* retry_count;     // number of entries appended
+  const long long* list;               // null: cells 0..n_cells-1; else the cells to process ...
+  const unsigned long long* list_count;  // ... and how many of them (device memory)
 };
 
 // status bits (mirror of include/kratos_chem.h, kept numeric so that device code needs no host header)
 #define KR_DST_REJECTED 1
 #define KR_DST_CLAMPED_NEG 2
+#define KR_DST_FP64_FALLBACK 4
 #define KR_DST_FAILED 8
 #define KR_DST_T_CLAMPED 16
 #define KR_DST_NO_RESERVOIR 32

@@ -1,0 +1,852 @@
+// kr_wpc.cuh -- warp-per-cell solve kernel with the per-cell matrix in REGISTERS (13 <= N <= 64 in fp64; any
+// N <= 64 in mixed precision).  Compiled at kr_network_create (NVRTC, sm_100a) with the sizes of the network
+// as macros, so every register tile is exactly as large as the network needs:
+//   KRW_N KRW_S KRW_R KRW_E KRW_ENERGY KRW_ANY_REV KRW_ANY_TB KRW_ANY_QEXT KRW_NAUX    the network
+//   KRW_W      warps per cell (1 or 2)         KRW_TR  row groups inside a warp (4 or 8; TC = 32 / TR)
+//   KRW_RB     rows per thread (TR RB >= N)    KRW_CB  columns per thread (TC W CB >= N + 1)
+//   KRW_MIXED  0: fp64 throughout   1: fp32 matrix + elimination, fp64 residuals, iterative refinement (R15)
+//   KRW_CPB    cells per block                 KRW_MIN_BLOCKS  launch bound
+//
+// Work split of one Newton iteration (DESIGN.md steps 2-7) inside the group of 32 W threads that owns a cell:
+//   thermo            : thread <-> species
+//   rate constants, q : thread <-> reaction
+//   Jacobian          : thread <-> COLUMN m, each dq_r/dn_m formed once by the column's owner and scattered down
+//                       the column in shared memory: no atomics (replaces PAPER.md:232), eq. 19 / eq. 20
+//   elimination       : the matrix [I - hJ | -G] is spread over the threads as a TR x (TC W) grid of RB x CB
+//                       REGISTER tiles (rows blocked, columns cyclic).  Column k: scaled-pivot search among the
+//                       not yet used rows by the TR lanes that hold the column (shuffles), multipliers and the
+//                       pivot row published through shared memory, rank-1 update of every tile -- RB x CB
+//                       independent FMAs per thread and step against RB + CB shared-memory loads.  Rows are never
+//                       exchanged (implicit pivoting: a used row is marked); the update is applied to the used
+//                       rows as well (Gauss-Jordan form of Algorithm 1's elimination), which
+//                       removes the serial back substitution: after N columns row p_k holds x_k * pivot_k.
+//   mixed precision   : J is assembled in fp32, rows are scaled to unit max-norm, the elimination runs in fp32 and
+//                       its multipliers are kept (N^2 floats in the space J occupied); the linear residual
+//                       r = -G - (I - hJ) d is formed in fp64 WITHOUT a stored fp64 matrix (J d is the analytic
+//                       directional derivative, one pass over the reactions) and the correction is obtained by
+//                       replaying the kept multipliers on r -- refinement until the correction is far below the
+//                       Newton tolerance.
+// Controller scalars are replicated in every thread and evolve identically.  Persistent: a group that finishes a
+// cell pulls the next one from the global counter (a8).
+#pragma once
+#include "kr_tables.h"
+#include "kr_math.cuh"
+
+#ifndef KRW_REF_MAX
+#define KRW_REF_MAX 5          // most refinement passes per Newton iteration (mixed mode)
+#endif
+
+namespace krw {
+
+constexpr int N = KRW_N, S = KRW_S, R = KRW_R, E = KRW_E;
+constexpr int W = KRW_W, GT = 32 * KRW_W;
+constexpr int TR = KRW_TR, TC = 32 / KRW_TR, RB = KRW_RB, CB = KRW_CB;
+constexpr int NCG = TC * W;                 // column groups; column c belongs to group c % NCG, local index c / NCG
+constexpr int LD = (N + 1) | 1;             // leading dimension of J in shared memory (elements)
+constexpr int LTS = TR * RB + TR;           // stride of one multiplier vector (one pad element per row group)
+constexpr bool ENERGY = KRW_ENERGY != 0, MIXED = KRW_MIXED != 0;
+static_assert(TR * RB >= N, "row tiles do not cover N");
+static_assert(NCG * CB >= N + 1, "column tiles do not cover N + 1");
+static_assert(W == 1 || W == 2, "one or two warps per cell");
+
+#if KRW_MIXED
+typedef float MT;
+#else
+typedef double MT;
+#endif
+
+// ---- shared memory of one cell (byte offsets, all 8-byte aligned) ------------------------------------------------
+constexpr int a8(int x) { return (x + 7) & ~7; }
+constexpr int MAT_ELEMS = N * ((MIXED && LTS > LD) ? LTS : LD);   // J, later (mixed) the N multiplier vectors
+constexpr int oU = 0;                                   // double[N]  iterate u^{k-1}
+constexpr int oUN = oU + 8 * N;                         // double[N]  last accepted state
+constexpr int oF = oUN + 8 * N;                         // double[N]  f(u)
+constexpr int oB = oF + 8 * N;                          // double[N]  -G
+constexpr int oX = oB + 8 * N;                          // double[N]  Newton update delta
+constexpr int oRS = oX + 8 * N;                         // double[N]  residual of the linear system (mixed)
+constexpr int oVI = oRS + 8 * N;                        // double[N]  1 / row scale
+constexpr int oTH = oVI + 8 * N;                        // double[3S] ghat, uhat, chat
+constexpr int oKF = oTH + 8 * 3 * S;                    // double[R]
+constexpr int oKR = oKF + 8 * R;                        // double[R]
+constexpr int oQ = oKR + 8 * R;                         // double[R]  q_r, later dq_r (mixed refinement)
+constexpr int oDQT = oQ + 8 * R;                        // double[R]  dq_r/dT (energy)
+constexpr int oQH = oDQT + (ENERGY ? 8 * R : 0);        // double[R]  k_f P' - k_r P'' (third body)
+constexpr int oMT = oQH + (KRW_ANY_TB ? 8 * R : 0);     // double[R]  M_r
+constexpr int oRED = oMT + (KRW_ANY_TB ? 8 * R : 0);    // double[8 W + 4] reduction scratch, cell slot, scalars
+constexpr int oRP = oRED + 8 * (8 * W + 4);             // MT[N]      reciprocal pivots
+constexpr int oUR = a8(oRP + int(sizeof(MT)) * N);      // MT[NCG CB] pivot row
+constexpr int oLK = a8(oUR + int(sizeof(MT)) * NCG * CB);   // MT[2 LTS] multipliers of the current column (fp64 mode)
+constexpr int oKOF = a8(oLK + int(sizeof(MT)) * 2 * LTS);   // int[TR RB] column in which row i was the pivot row
+constexpr int oPOF = a8(oKOF + 4 * TR * RB);            // int[N]     pivot row of column k
+constexpr int oPIV = a8(oPOF + 4 * N);                  // int[2]     pivot row of the current column (double buffered)
+constexpr int oMAT = a8(oPIV + 8);                      // MT[MAT_ELEMS]
+constexpr int CELL_BYTES = a8(oMAT + int(sizeof(MT)) * MAT_ELEMS);
+
+#ifdef KRW_CELL_BYTES
+static_assert(CELL_BYTES == KRW_CELL_BYTES, "host and device disagree on the shared-memory layout");
+#endif
+
+struct Cell {
+  char* base;
+  __device__ __forceinline__ double* d(int off) const { return reinterpret_cast<double*>(base + off); }
+  __device__ __forceinline__ MT* m(int off) const { return reinterpret_cast<MT*>(base + off); }
+  __device__ __forceinline__ int* i(int off) const { return reinterpret_cast<int*>(base + off); }
+};
+
+// ---- the group of 32 W threads -----------------------------------------------------------------------------------
+struct Grp {
+  double* red;   // [8 W + 4]
+  int g, gl;     // group index in the block, thread index in the group
+  __device__ __forceinline__ void sync() const {
+    if (W == 1) __syncwarp();
+    else asm volatile("bar.sync %0, %1;" ::"r"(g + 1), "r"(32 * W) : "memory");
+  }
+  template <int NV>
+  __device__ __forceinline__ void sum(double (&x)[NV]) const {     // fixed order: butterfly, then warps in index order
+#pragma unroll
+    for (int i = 0; i < NV; ++i)
+      for (int off = 16; off > 0; off >>= 1) x[i] += __shfl_xor_sync(0xffffffffu, x[i], off);
+    if (W > 1) {
+      const int w = gl >> 5;
+      if ((gl & 31) == 0)
+        for (int i = 0; i < NV; ++i) red[w * NV + i] = x[i];
+      sync();
+#pragma unroll
+      for (int i = 0; i < NV; ++i) {
+        double s = red[i];
+        for (int ww = 1; ww < W; ++ww) s += red[ww * NV + i];
+        x[i] = s;
+      }
+      sync();
+    }
+  }
+  __device__ __forceinline__ double max(double x) const {          // NaN-dropping, the oracle's "if (x > m) m = x"
+    for (int off = 16; off > 0; off >>= 1) { const double y = __shfl_xor_sync(0xffffffffu, x, off); x = (y > x) ? y : x; }
+    if (W > 1) {
+      const int w = gl >> 5;
+      if ((gl & 31) == 0) red[w] = x;
+      sync();
+      double m = red[0];
+      for (int ww = 1; ww < W; ++ww) { const double y = red[ww]; m = (y > m) ? y : m; }
+      x = m;
+      sync();
+    }
+    return x;
+  }
+  __device__ __forceinline__ double min(double x) const { return -max(-x); }
+  __device__ __forceinline__ bool all(bool p) const {
+    int ok = __all_sync(0xffffffffu, p);
+    if (W > 1) {
+      const int w = gl >> 5;
+      if ((gl & 31) == 0) red[w] = ok ? 1.0 : 0.0;
+      sync();
+      ok = 1;
+      for (int ww = 0; ww < W; ++ww) ok = ok && (red[ww] != 0.0);
+      sync();
+    }
+    return ok != 0;
+  }
+};
+
+__device__ __forceinline__ double ipow(double x, int e) {          // e in 0..3 (R20)
+  double p = 1.0;
+  if (e >= 1) p = x;
+  if (e >= 2) p *= x;
+  if (e >= 3) p *= x;
+  return p;
+}
+__device__ __forceinline__ bool finite(double x) { return fabs(x) <= 1.79769313486231570e308; }
+__device__ __forceinline__ MT mt_rcp(MT x) {
+#if KRW_MIXED
+  return __frcp_rn(x);
+#else
+  return krs_rcp(x);
+#endif
+}
+
+// ---- steps 2-3: thermo, thread <-> species (R7) --------------------------------------------------
+__device__ __forceinline__ void thermo(const KrNetDev& n, const Cell& c, const Grp& G, double T, double invT, double lnT) {
+  double* TH = c.d(oTH);
+  const double T2 = T * T, T3 = T2 * T, T4 = T3 * T;
+  for (int s = G.gl; s < S; s += GT) {
+    const double* a = n.nasa + 14 * s + ((T <= n.T_mid[s]) ? 0 : 7);
+    const double a0 = a[0], a1 = a[1], a2 = a[2], a3 = a[3], a4 = a[4], a5 = a[5], a6 = a[6];
+    const double cp = a0 + a1 * T + a2 * T2 + a3 * T3 + a4 * T4;
+    const double h = a0 + a1 * T * 0.5 + a2 * T2 * (1.0 / 3.0) + a3 * T3 * 0.25 + a4 * T4 * 0.2 + a5 * invT;
+    const double sR = a0 * lnT + a1 * T + a2 * T2 * 0.5 + a3 * T3 * (1.0 / 3.0) + a4 * T4 * 0.25 + a6;
+    TH[s] = h - sR; TH[S + s] = h - 1.0; TH[2 * S + s] = cp - 1.0;
+  }
+}
+
+// ---- steps 3-4: thread <-> reaction.  Rate constants (eq. 16 with R4, detailed balance R5, unary R16/R17) when
+// computeK, then q_r, dq_r/dT, and the third-body factors.  Returns partial sums of (q_ext/k_B) q and (q_ext/k_B) dq/dT.
+__device__ __forceinline__ void reactions(const KrNetDev& n, const Cell& c, const Grp& G, double Ncal, double invT, double lnT,
+                                          double aux0, const double* __restrict__ aux, long long cell, long long n_cells,
+                                          bool computeK, double& heat_sum, double& heat_dT) {
+  double *U = c.d(oU), *TH = c.d(oTH), *KF = c.d(oKF), *KR = c.d(oKR), *Q = c.d(oQ);
+  heat_sum = 0.0; heat_dT = 0.0;
+  for (int r = G.gl; r < R; r += GT) {
+    const int fl = n.flags[r];
+    int sp[6], nu[6];
+#pragma unroll
+    for (int k = 0; k < 6; ++k) { sp[k] = n.sp[6 * r + k]; nu[k] = n.nu[6 * r + k]; }
+    double kf, kr = 0.0, dlf = 0.0, dlr = 0.0;
+    if (computeK) {
+      if (fl & KR_DF_CONST) kf = n.A[r];
+      else if (fl & KR_DF_AUX) {
+        const int ai = n.auxi[r];
+        kf = n.A[r] * (ai > 0 ? aux[(long long)ai * n_cells + cell] : aux0);
+      } else {
+        const double beta = n.beta[r], Ea = n.Ea[r];
+        const double lnkf = n.c0[r] + beta * lnT - Ea * invT;
+        kf = krs_exp(lnkf);
+        dlf = (beta + Ea * invT) * invT;
+        if (fl & KR_DF_REV) {
+          double sg = 0.0, su = 0.0;
+#pragma unroll
+          for (int k = 0; k < 6; ++k)
+            if (sp[k] >= 0) {
+              const double cf = (k < 3) ? -(double)nu[k] : (double)nu[k];
+              sg += cf * TH[sp[k]];
+              su += cf * TH[S + sp[k]];
+            }
+          const double lnKc = -sg + (double)n.dnu_tot[r] * (n.ln_p0_kB - lnT);
+          kr = krs_exp(lnkf - lnKc);
+          dlr = dlf - su * invT;
+        }
+      }
+      KF[r] = kf; KR[r] = kr;
+    } else {
+      kf = KF[r]; kr = KR[r];
+    }
+    double Pf = 1.0, Pr = 1.0;
+#pragma unroll
+    for (int k = 0; k < 6; ++k)
+      if (sp[k] >= 0) {
+        const double p = ipow(Ncal * U[sp[k]], nu[k]);
+        if (k < 3) Pf *= p; else Pr *= p;
+      }
+    double Mtb = 1.0;
+    const double qhat = kf * Pf - kr * Pr;
+    if (KRW_ANY_TB && (fl & KR_DF_TB)) {
+      Mtb = 0.0;
+      for (int s = 0; s < S; ++s) Mtb += n.tb_eff[r * S + s] * (Ncal * U[s]);
+      c.d(oQH)[r] = qhat; c.d(oMT)[r] = Mtb;
+    }
+    const double q = Mtb * qhat;
+    Q[r] = q;
+    const double qk = KRW_ANY_QEXT ? n.qk[r] : 0.0;
+    heat_sum += qk * q;
+    if (ENERGY) {
+      const double dqdT = Mtb * (kf * dlf * Pf - kr * dlr * Pr);
+      c.d(oDQT)[r] = dqdT;
+      heat_dT += qk * dqdT;
+    }
+  }
+}
+
+// ---- f rows (and the T column of J when wantJ): thread <-> species row, gather in reaction order (eq. 15, eq. 20)
+__device__ __forceinline__ void rows(const KrNetDev& n, const Cell& c, const Grp& G, double invN, bool wantJ) {
+  double *Q = c.d(oQ), *F = c.d(oF);
+  MT* J = c.m(oMAT);
+  for (int s = G.gl; s < S; s += GT) {
+    double ys = 0.0, jt = 0.0;
+    const int p1 = n.row_ptr[s + 1];
+    for (int p = n.row_ptr[s]; p < p1; ++p) {
+      const int ent = n.row_ent[p];
+      const int r = ent >> 8;
+      const double dnu = (double)((ent & 255) - 128);
+      ys += dnu * Q[r];
+      if (ENERGY) jt += dnu * c.d(oDQT)[r];
+    }
+    F[s] = ys * invN;
+    if (ENERGY && wantJ) J[s * LD + S] = (MT)(jt * invN);
+  }
+}
+
+// ---- Jacobian columns (eq. 19): thread <-> column m.  invC = 1 / sum_s y_s chat_s (energy equation only).
+__device__ __forceinline__ void columns(const KrNetDev& n, const Cell& c, const Grp& G, double Ncal, double T, double invC) {
+  double *U = c.d(oU), *TH = c.d(oTH), *KF = c.d(oKF), *KR = c.d(oKR);
+  MT* J = c.m(oMAT);
+  for (int m = G.gl; m < S; m += GT) {
+    for (int i = 0; i < N; ++i) J[i * LD + m] = (MT)0;
+    double heat_dn = 0.0;
+    const double nm = Ncal * U[m];
+    const int p1 = n.col_ptr[m + 1];
+    for (int p = n.col_ptr[m]; p < p1; ++p) {
+      const int ent = n.col_ent[p];
+      const int r = ent >> 4, slot = ent & 15;
+      int sp[6], nu[6];
+#pragma unroll
+      for (int k = 0; k < 6; ++k) { sp[k] = n.sp[6 * r + k]; nu[k] = n.nu[6 * r + k]; }
+      double d;
+      if (slot < 6) {
+        const int base = (slot < 3) ? 0 : 3;
+        double others = 1.0;
+        int e = 1;
+#pragma unroll
+        for (int k = 0; k < 6; ++k) {
+          if (k == slot) e = nu[k];
+          else if (k >= base && k < base + 3 && sp[k] >= 0) others *= ipow(Ncal * U[sp[k]], nu[k]);
+        }
+        const double kk2 = (slot < 3) ? KF[r] : -KR[r];
+        const double Mtb = (KRW_ANY_TB && (n.flags[r] & KR_DF_TB)) ? c.d(oMT)[r] : 1.0;
+        d = Mtb * (kk2 * (double)e * ipow(nm, e - 1) * others);
+      } else {
+        d = n.tb_eff[r * S + m] * c.d(oQH)[r];
+      }
+#pragma unroll
+      for (int k = 0; k < 6; ++k)
+        if (sp[k] >= 0) J[sp[k] * LD + m] += (MT)(((k < 3) ? -(double)nu[k] : (double)nu[k]) * d);
+      if (ENERGY && KRW_ANY_QEXT) heat_dn += n.qk[r] * d;
+    }
+    if (ENERGY) {
+      double acc = 0.0;
+      for (int s = 0; s < S; ++s) acc += TH[S + s] * (double)J[s * LD + m];
+      J[S * LD + m] = (MT)((heat_dn - T * acc) * invC);
+    }
+  }
+}
+
+// ---- full evaluation of f (and J) at U.  Thermo / KF / KR valid as the flags say.  Leaves 1/C and sum_s chat_s f_s
+// in the scalar slots (used by the matrix-free product of the mixed mode).
+__device__ __forceinline__ void eval(const KrNetDev& n, const Cell& c, const Grp& G, double Ncal, double T, double aux0,
+                                     const double* __restrict__ aux, long long cell, long long n_cells, bool computeK,
+                                     bool wantJ) {
+  const double invT = krs_rcp(T), lnT = (ENERGY || computeK) ? log(T) : 0.0;
+  const double invN = krs_rcp(Ncal);
+  double *U = c.d(oU), *TH = c.d(oTH), *F = c.d(oF);
+  double red[3];
+  reactions(n, c, G, Ncal, invT, lnT, aux0, aux, cell, n_cells, computeK, red[0], red[1]);
+  red[2] = 0.0;
+  if (ENERGY) {
+    for (int s = G.gl; s < S; s += GT) red[2] += U[s] * TH[2 * S + s];
+    G.sum(red);
+  }
+  G.sync();
+  const double heat_sum = red[0], heat_dT = red[1];
+  const double invC = ENERGY ? krs_rcp(red[2]) : 1.0;
+  rows(n, c, G, invN, wantJ);
+  if (wantJ) columns(n, c, G, Ncal, T, invC);
+  G.sync();
+  if (ENERGY) {
+    MT* J = c.m(oMAT);
+    double r2[3] = {0.0, 0.0, 0.0};
+    for (int s = G.gl; s < S; s += GT) {
+      const double fs = F[s], uh = TH[S + s];
+      r2[0] += uh * fs;
+      r2[1] += TH[2 * S + s] * fs;
+      if (wantJ) r2[2] += uh * (double)J[s * LD + S];
+    }
+    G.sum(r2);
+    if (G.gl == 0) {
+      F[S] = (heat_sum * invN - T * r2[0]) * invC;
+      if (wantJ) J[S * LD + S] = (MT)((heat_dT * invN - T * r2[2] - r2[1]) * invC);
+      G.red[8 * W + 1] = invC; G.red[8 * W + 2] = r2[1];
+    }
+    G.sync();
+  }
+}
+
+#if KRW_MIXED
+// ---- mixed mode: RS = B - (I - hJ) X in fp64 without a stored fp64 matrix.  J X is the analytic directional
+// derivative of f along X with exactly the terms of DESIGN.md step 5: per reaction
+//   dq_r = M_r sum_slots (k e n^(e-1) prod others) dn_slot + (third body) qhat_r sum_s eff_s dn_s + (dq_r/dT) dT,
+// then (J X)_s = (1/Ncal) sum_r dnu_rs dq_r and (J X)_T = [ (1/Ncal) sum_r (q_ext/k_B) dq_r - T sum_s uhat_s (J X)_s
+// - (sum_s chat_s f_s) dT ] / C.
+__device__ __forceinline__ void residual(const KrNetDev& n, const Cell& c, const Grp& G, double Ncal, double T, double h) {
+  double *U = c.d(oU), *TH = c.d(oTH), *KF = c.d(oKF), *KR = c.d(oKR), *DQ = c.d(oQ), *X = c.d(oX), *B = c.d(oB),
+         *RS = c.d(oRS);
+  const double invN = krs_rcp(Ncal);
+  const double dT = ENERGY ? X[S] : 0.0;
+  double red[2] = {0.0, 0.0};
+  for (int r = G.gl; r < R; r += GT) {
+    int sp[6], nu[6];
+#pragma unroll
+    for (int k = 0; k < 6; ++k) { sp[k] = n.sp[6 * r + k]; nu[k] = n.nu[6 * r + k]; }
+    const int fl = n.flags[r];
+    const double kf = KF[r], kr = KR[r];
+    double nn[6];
+#pragma unroll
+    for (int k = 0; k < 6; ++k) nn[k] = (sp[k] >= 0) ? Ncal * U[sp[k]] : 1.0;
+    double dq = 0.0;
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+      if (sp[k] < 0) continue;
+      if (k >= 3 && !(fl & KR_DF_REV)) continue;
+      const int base = (k < 3) ? 0 : 3;
+      double others = 1.0;
+#pragma unroll
+      for (int kk = 0; kk < 3; ++kk)
+        if (base + kk != k && sp[base + kk] >= 0) others *= ipow(nn[base + kk], nu[base + kk]);
+      const double kk2 = (k < 3) ? kf : -kr;
+      dq += kk2 * (double)nu[k] * ipow(nn[k], nu[k] - 1) * others * (Ncal * X[sp[k]]);
+    }
+    if (KRW_ANY_TB && (fl & KR_DF_TB)) {
+      double dM = 0.0;
+      for (int s = 0; s < S; ++s) dM += n.tb_eff[r * S + s] * (Ncal * X[s]);
+      dq = c.d(oMT)[r] * dq + c.d(oQH)[r] * dM;
+    }
+    if (ENERGY) dq += c.d(oDQT)[r] * dT;
+    DQ[r] = dq;
+    if (ENERGY && KRW_ANY_QEXT) red[0] += n.qk[r] * dq;
+  }
+  G.sync();
+  for (int s = G.gl; s < S; s += GT) {
+    double js = 0.0;
+    const int p1 = n.row_ptr[s + 1];
+    for (int p = n.row_ptr[s]; p < p1; ++p) {
+      const int ent = n.row_ent[p];
+      js += (double)((ent & 255) - 128) * DQ[ent >> 8];
+    }
+    js *= invN;
+    RS[s] = B[s] - (X[s] - h * js);
+    if (ENERGY) red[1] += TH[S + s] * js;
+  }
+  if (ENERGY) {
+    G.sum(red);
+    if (G.gl == 0) {
+      const double invC = G.red[8 * W + 1], scf = G.red[8 * W + 2];
+      const double jT = (red[0] * invN - T * red[1] - scf * dT) * invC;
+      RS[S] = B[S] - (dT - h * jT);
+    }
+  }
+  G.sync();
+}
+#endif
+
+// ---- step 7: elimination of [I - hJ | -G] in register tiles ------------------------------------------------------
+struct Lane {
+  int lane, wq, tr, tc, cg;
+  __device__ __forceinline__ explicit Lane(int gl) : lane(gl & 31), wq(gl >> 5), tr((gl & 31) / TC), tc((gl & 31) % TC),
+                                                     cg((gl >> 5) * TC + (gl & 31) % TC) {}
+};
+__device__ __forceinline__ int lidx(int row) { return row + row / RB; }     // padded index into a multiplier vector
+
+template <int I>
+__device__ __forceinline__ void publish_row(const MT (&a)[RB][CB], int kb, MT* UR, int cg) {
+#pragma unroll
+  for (int j = 0; j < CB; ++j)
+    if (j >= kb) UR[j * NCG + cg] = a[I][j];
+}
+
+#define KRW_PUB_CASE(I) \
+  case I: if constexpr (I < RB) publish_row<(I < RB ? I : 0)>(a, kb, UR, L.cg); break;
+
+// Pass A (thread <-> row): B = -(U - UN - h F), row scales of I - hJ.  Pass B: tiles.  Then N elimination columns.
+// On success X holds the solution of (I - hJ) X = B; in mixed mode the multipliers, reciprocal pivots and the row
+// order stay in shared memory for replay().  Uniform return value (false: zero row, non-finite entry or no pivot).
+__device__ __forceinline__ bool eliminate(const Cell& c, const Grp& G, double h) {
+  const Lane L(G.gl);
+  double *U = c.d(oU), *UN = c.d(oUN), *F = c.d(oF), *B = c.d(oB), *VI = c.d(oVI), *X = c.d(oX);
+  MT* J = c.m(oMAT);
+  const MT hm = (MT)h;
+  bool rows_ok = true;
+  for (int i = G.gl; i < N; i += GT) {
+    B[i] = -(U[i] - UN[i] - h * F[i]);
+    MT big = (MT)0;
+    for (int j = 0; j < N; ++j) {
+      const MT x = ((i == j) ? (MT)1 : (MT)0) - hm * J[i * LD + j];
+      const MT ax = fabs(x);
+      big = (ax > big) ? ax : big;
+      if (!(ax <= (MT)(MIXED ? 3.0e38 : 1.7e308))) big = ax;      // keep inf / NaN: the row is refused below
+    }
+    const bool ok = (big > (MT)(MIXED ? 1e-30 : 1e-300)) && (big <= (MT)(MIXED ? 3.0e38 : 1.7e308));
+    rows_ok = rows_ok && ok;
+    VI[i] = ok ? 1.0 / (double)big : 0.0;
+  }
+  rows_ok = G.all(rows_ok);
+  G.sync();
+  if (!rows_ok) return false;
+
+  MT a[RB][CB];
+#if !KRW_MIXED
+  double vinv[RB];
+#endif
+  unsigned alive = 0;
+#pragma unroll
+  for (int i = 0; i < RB; ++i) {
+    const int row = L.tr * RB + i;
+    const bool rin = row < N;
+    const double vi = rin ? VI[row] : 0.0;
+#if !KRW_MIXED
+    vinv[i] = vi;
+#endif
+    if (rin) alive |= 1u << i;
+#pragma unroll
+    for (int j = 0; j < CB; ++j) {
+      const int col = j * NCG + L.cg;
+      MT x = (MT)0;
+      if (rin && col < N) {
+        x = ((row == col) ? (MT)1 : (MT)0) - hm * J[row * LD + col];
+        if (MIXED) x *= (MT)vi;
+      } else if (rin && col == N) {
+        x = MIXED ? (MT)(B[row] * vi) : (MT)B[row];
+      }
+      a[i][j] = x;
+    }
+  }
+  G.sync();                                   // J is dead from here on: the mixed mode reuses its space
+
+  MT* UR = c.m(oUR);
+  MT* RP = c.m(oRP);
+  int* PIV = c.i(oPIV);
+  int* KOF = c.i(oKOF);
+#pragma unroll
+  for (int kb = 0; kb < CB; ++kb) {
+    for (int kc = 0; kc < NCG; ++kc) {
+      const int k = kb * NCG + kc;
+      if (k >= N) break;
+      MT* Lk = MIXED ? (c.m(oMAT) + k * LTS) : (c.m(oLK) + (k & 1) * LTS);
+      if (W == 1 || L.wq == kc / TC) {        // the warp that holds column k: scaled pivot search (Algorithm 1)
+        MT best = (MT)-1, pv = (MT)0;
+        int bi = -1;
+#pragma unroll
+        for (int i = 0; i < RB; ++i) {
+#if KRW_MIXED
+          const MT t = fabsf(a[i][kb]);
+#else
+          const MT t = fabs(a[i][kb]) * vinv[i];
+#endif
+          if (((alive >> i) & 1u) && t > best) { best = t; pv = a[i][kb]; bi = L.tr * RB + i; }
+        }
+#pragma unroll
+        for (int off = TC; off < 32; off <<= 1) {
+          const MT t2 = __shfl_xor_sync(0xffffffffu, best, off);
+          const MT p2 = __shfl_xor_sync(0xffffffffu, pv, off);
+          const int i2 = __shfl_xor_sync(0xffffffffu, bi, off);
+          if (i2 >= 0 && (bi < 0 || t2 > best || (t2 == best && i2 < bi))) { best = t2; pv = p2; bi = i2; }
+        }
+        if (L.tc == kc % TC) {
+          const bool okp = (bi >= 0) && (fabs(pv) >= (MT)(MIXED ? 1e-30 : 1e-300));
+          const MT rp = mt_rcp(okp ? pv : (MT)1);
+#pragma unroll
+          for (int i = 0; i < RB; ++i) {
+            const int row = L.tr * RB + i;
+            Lk[row + L.tr] = (row == bi) ? (MT)0 : a[i][kb] * rp;
+          }
+          if (L.tr == 0) { PIV[k & 1] = okp ? bi : -1; RP[k] = rp; }
+        }
+      }
+      G.sync();
+      const int p = PIV[k & 1];
+      if (p < 0) return false;
+      const int trp = p / RB, ip = p - trp * RB;
+      if (L.tr == trp) {                      // the lanes that hold row p publish it and retire it
+        switch (ip) {
+          KRW_PUB_CASE(0) KRW_PUB_CASE(1) KRW_PUB_CASE(2) KRW_PUB_CASE(3) KRW_PUB_CASE(4) KRW_PUB_CASE(5) KRW_PUB_CASE(6)
+          KRW_PUB_CASE(7) KRW_PUB_CASE(8) KRW_PUB_CASE(9) KRW_PUB_CASE(10) KRW_PUB_CASE(11) KRW_PUB_CASE(12)
+          KRW_PUB_CASE(13) KRW_PUB_CASE(14) KRW_PUB_CASE(15) KRW_PUB_CASE(16) KRW_PUB_CASE(17) KRW_PUB_CASE(18)
+          KRW_PUB_CASE(19) KRW_PUB_CASE(20) KRW_PUB_CASE(21)
+          default: break;
+        }
+        alive &= ~(1u << ip);
+        if (L.cg == 0) { KOF[p] = k; c.i(oPOF)[k] = p; }
+      }
+      __syncwarp();
+      MT l[RB], u[CB];
+#pragma unroll
+      for (int i = 0; i < RB; ++i) l[i] = Lk[L.tr * RB + i + L.tr];
+#pragma unroll
+      for (int j = 0; j < CB; ++j)
+        if (j >= kb) u[j] = UR[j * NCG + L.cg];
+      if (L.cg <= kc) u[kb] = (MT)0;          // columns <= k of this block are finished
+#pragma unroll
+      for (int j = 0; j < CB; ++j)
+        if (j >= kb) {
+#pragma unroll
+          for (int i = 0; i < RB; ++i) a[i][j] = fma(-l[i], u[j], a[i][j]);
+        }
+    }
+  }
+  G.sync();
+  constexpr int jN = N / NCG, cgN = N % NCG;  // the right-hand-side column
+  if (L.cg == cgN) {
+#pragma unroll
+    for (int i = 0; i < RB; ++i) {
+      const int row = L.tr * RB + i;
+      if (row < N) { const int k = KOF[row]; X[k] = (double)a[i][jN] * (double)RP[k]; }
+    }
+  }
+  G.sync();
+  return true;
+}
+#undef KRW_PUB_CASE
+
+#if KRW_MIXED
+// ---- mixed mode: correction d = (I - hJ)^-1 RS from the kept multipliers (2 N^2 fp32 flops), X += d.
+// Each warp replays all rows (lane <-> rows lane, lane + 32): no traffic between warps.  Returns the weighted
+// max-norms of the correction and of the corrected update, in units of the Newton tolerance (step 6's e_k).
+__device__ __forceinline__ void replay(const Cell& c, const Grp& G, const KrOptsDev& o, double& wD, double& wX) {
+  constexpr int NRL = (N + 31) / 32;
+  const int lane = G.gl & 31;
+  double *RS = c.d(oRS), *VI = c.d(oVI), *X = c.d(oX), *U = c.d(oU);
+  const MT* LT = c.m(oMAT);
+  const MT* RP = c.m(oRP);
+  const int *POF = c.i(oPOF), *KOF = c.i(oKOF);
+  float r[NRL];
+#pragma unroll
+  for (int q = 0; q < NRL; ++q) {
+    const int row = lane + 32 * q;
+    r[q] = (row < N) ? (float)(RS[row] * VI[row]) : 0.0f;
+  }
+  for (int k = 0; k < N; ++k) {
+    const int p = POF[k];
+    float mine = r[0];
+#pragma unroll
+    for (int q = 1; q < NRL; ++q) mine = ((p >> 5) == q) ? r[q] : mine;
+    const float rp = __shfl_sync(0xffffffffu, mine, p & 31);
+#pragma unroll
+    for (int q = 0; q < NRL; ++q) {
+      const int row = lane + 32 * q;
+      if (row < N) r[q] = fmaf(-LT[k * LTS + lidx(row)], rp, r[q]);
+    }
+  }
+  double xn[NRL];
+  int kk[NRL];
+  double wd = 0.0, wx = 0.0;
+#pragma unroll
+  for (int q = 0; q < NRL; ++q) {
+    const int row = lane + 32 * q;
+    kk[q] = -1; xn[q] = 0.0;
+    if (row < N) {
+      const int k = KOF[row];
+      const double d = (double)(r[q] * RP[k]);
+      const double x = X[k] + d;
+      const double wgt = o.rtol * fabs(U[k] + x) + ((k < S) ? o.atol_y : o.atol_T);
+      const double a = fabs(d) / wgt, b = fabs(x) / wgt;
+      wd = (a > wd || !(a == a)) ? a : wd;      // NaN sticks
+      wx = (b > wx) ? b : wx;
+      kk[q] = k; xn[q] = x;
+    }
+  }
+  for (int off = 16; off > 0; off >>= 1) {
+    const double y = __shfl_xor_sync(0xffffffffu, wd, off); wd = (y > wd || !(y == y)) ? y : wd;
+    const double z = __shfl_xor_sync(0xffffffffu, wx, off); wx = (z > wx) ? z : wx;
+  }
+  if (W > 1) G.sync();                         // every warp has read X
+  if (G.gl < 32) {
+#pragma unroll
+    for (int q = 0; q < NRL; ++q)
+      if (kk[q] >= 0) X[kk[q]] = xn[q];
+  }
+  G.sync();
+  wD = wd; wX = wx;
+}
+#endif
+
+}  // namespace krw
+
+extern "C" __global__ void __launch_bounds__(32 * KRW_W * KRW_CPB, KRW_MIN_BLOCKS)
+kr_wpc_kernel(const KrNetDev n, const KrOptsDev o, const KrStepArgs a) {
+  using namespace krw;
+  extern __shared__ __align__(16) char kr_sm_raw[];
+  const int K = o.max_newton;
+  Grp G;
+  G.g = threadIdx.x / GT; G.gl = threadIdx.x % GT;
+  Cell c;
+  c.base = kr_sm_raw + (size_t)G.g * CELL_BYTES;
+  G.red = c.d(oRED);
+  volatile long long* cellslot = (volatile long long*)(c.d(oRED) + 8 * W);
+  double *U = c.d(oU), *UN = c.d(oUN), *F = c.d(oF), *X = c.d(oX);
+
+  unsigned long long c_acc = 0, c_rej = 0, c_newton = 0, c_rate = 0, c_failed = 0, c_ref = 0;   // thread 0 of the group
+
+  for (;;) {
+    if (G.gl == 0) {
+      long long idx = (long long)atomicAdd(a.counter, 1ull);
+      if (a.list) idx = (idx < (long long)*a.list_count) ? a.list[idx] : a.n_cells;
+      *cellslot = idx;
+    }
+    G.sync();
+    const long long cell = *cellslot;
+    G.sync();
+    if (cell >= a.n_cells) break;
+
+    // ---- step 1: layout-in, clamp, first sub-step -------------------------------------------------
+    int st = a.list ? KR_DST_FP64_FALLBACK : 0;
+    double Tc = a.T[cell];
+    if (Tc < n.T_lo) { Tc = n.T_lo; st |= KR_DST_T_CLAMPED; }
+    if (Tc > n.T_hi) { Tc = n.T_hi; st |= KR_DST_T_CLAMPED; }
+    const double Ncal = a.rho[cell] * (1.0 / KR_M_U);
+    const double T_iso = Tc;
+    const double aux0 = (KRW_NAUX > 0) ? a.aux[cell] : 0.0;
+    for (int s = G.gl; s < S; s += GT) { const double x = a.y[cell * S + s]; UN[s] = x; U[s] = x; }
+    if (ENERGY && G.gl == 0) { UN[S] = Tc; U[S] = Tc; }
+    G.sync();
+    double t = 0.0, h = a.dt;
+    int n_acc = 0, n_rej = 0;
+    {
+      const double invT = krs_rcp(Tc), lnT = log(Tc);
+      if (!ENERGY) {
+        if (KRW_ANY_REV) { thermo(n, c, G, Tc, invT, lnT); G.sync(); }
+        if (o.h0_mode != 1) {          // rate constants only (the h0 evaluation below computes them as well)
+          double hs, hd;
+          reactions(n, c, G, Ncal, invT, lnT, aux0, a.aux, cell, a.n_cells, true, hs, hd);
+          G.sync();
+        }
+        c_rate++;
+      }
+      if (o.h0_mode == 1) {
+        if (ENERGY) { thermo(n, c, G, Tc, invT, lnT); G.sync(); c_rate++; }
+        eval(n, c, G, Ncal, Tc, aux0, a.aux, cell, a.n_cells, true, false);
+        double big = 0.0;
+        for (int s = G.gl; s < S; s += GT) {
+          const double x = fabs(F[s]) / (fabs(UN[s]) + o.y_floor);
+          big = (x > big) ? x : big;
+        }
+        big = G.max(big);
+        if (big > 0.0 && finite(big)) h = fmin(a.dt, o.eta / big);
+      }
+    }
+    const double h_floor = o.h_min_rel * fmin(h, a.dt);
+
+    // ---- sub-step loop (steps 6-8) -------------------------------------------------------------------------------
+    bool failed = false, handoff = false;
+    for (;;) {
+      const double rem = a.dt - t;
+      bool last = false;
+      if (h >= rem) { h = rem; last = true; }
+      if (h < h_floor || n_acc + n_rej > o.max_substeps) { failed = true; break; }
+      for (int i = G.gl; i < N; i += GT) U[i] = UN[i];
+      G.sync();
+      double e = __longlong_as_double(0x7ff0000000000000LL), e_prev = 0.0;
+      int it = K + 1;
+      bool ran = true;
+      for (int k = 1; k <= K; ++k) {
+        const double T = ENERGY ? U[S] : T_iso;
+        if (ENERGY) { thermo(n, c, G, T, krs_rcp(T), log(T)); G.sync(); c_rate++; }
+        eval(n, c, G, Ncal, T, aux0, a.aux, cell, a.n_cells, ENERGY, true);
+        c_newton++;
+        if (!eliminate(c, G, h)) { ran = false; if (MIXED) handoff = a.retry_list != nullptr; break; }
+#if KRW_MIXED
+        {                                        // iterative refinement on the fp64 residual of the linear system
+          bool done = false;
+          double wprev = __longlong_as_double(0x7ff0000000000000LL);
+          for (int ref = 0; ref < KRW_REF_MAX; ++ref) {
+            residual(n, c, G, Ncal, T, h);
+            double wD, wX;
+            replay(c, G, o, wD, wX);
+            c_ref++;
+            if (!(wD == wD) || !finite(wD)) break;
+            if (wD <= 1e-4 || wD <= 1e-9 * wX) { done = true; break; }
+            if (wD > 0.25 * wprev) break;          // not contracting: fp32 does not resolve this matrix
+            wprev = wD;
+          }
+          if (!done) { handoff = a.retry_list != nullptr; ran = false; break; }
+        }
+#endif
+        bool fin = true;
+        double en = 0.0;
+        for (int i = G.gl; i < N; i += GT) {
+          const double dl = X[i];
+          const double x = U[i] + dl;
+          U[i] = x;
+          fin = fin && finite(x);
+          const double w = fabs(dl) / (o.rtol * fabs(x) + ((i < S) ? o.atol_y : o.atol_T));
+          en = (w > en) ? w : en;
+        }
+        fin = G.all(fin);
+        G.sync();
+        if (!fin) { ran = false; break; }
+        e = G.max(en);
+        if (it == K + 1 && e <= 1.0) it = k;
+        if (!o.fixed_newton) {
+          if (e <= 1.0) break;
+          if (k >= 2 && e > o.bail_ratio * e_prev) { ran = false; break; }
+        }
+        e_prev = e;
+      }
+      if (handoff) break;
+      // step 8: accept / reject
+      bool ok = ran && (e <= 1.0);
+      if (ok) {
+        double miny = __longlong_as_double(0x7ff0000000000000LL);
+        for (int s = G.gl; s < S; s += GT) miny = fmin(miny, U[s]);
+        miny = G.min(miny);
+        if (!(miny >= -o.neg_tol)) ok = false;
+      }
+      if (ok && ENERGY) {
+        const double Tn = U[S];
+        if (!(Tn >= n.T_lo && Tn <= n.T_hi)) ok = false;
+      }
+      if (ok && finite(o.chg_max)) {
+        double chg = 0.0;
+        for (int i = G.gl; i < N; i += GT) {
+          const double den = (i < S) ? (fabs(UN[i]) + o.chg_floor) : UN[i];
+          chg = fmax(chg, fabs(U[i] - UN[i]) / den);
+        }
+        chg = G.max(chg);
+        if (!(chg <= o.chg_max)) ok = false;
+      }
+      if (ok) {
+        n_acc++;
+        for (int i = G.gl; i < N; i += GT) UN[i] = U[i];
+        G.sync();
+        if (last) break;
+        t = t + h;
+        if (it <= o.it_fast) h = h * o.grow_fast;
+        else if (it <= o.it_mid) h = h * o.grow_mid;
+      } else {
+        n_rej++;
+        st |= KR_DST_REJECTED;
+        h = h * o.shrink;
+        G.sync();
+      }
+    }
+    if (handoff) {            // the caller's buffers were never written: the fp64 kernel redoes this cell from its input
+      if (G.gl == 0) a.retry_list[atomicAdd(a.retry_count, 1ull)] = cell;
+      G.sync();
+      continue;
+    }
+    c_acc += n_acc; c_rej += n_rej;
+    if (failed) {                                                 // R13: revert (the caller's buffers were never written)
+      c_failed++;
+      if (a.status && G.gl == 0) a.status[cell] = st | KR_DST_FAILED;
+      G.sync();
+      continue;
+    }
+    // ---- step 9: finalise (PAPER.md:212-216 stages 1-2; serial in thread 0, O(E S) once per cell) + layout-out -------
+    if (o.finalize && G.gl == 0) {
+      double* RW = c.d(oB);
+      bool any = false;
+      for (int nu = 0; nu < E; ++nu) {
+        double rem = 0.0;
+        for (int s = 0; s < S; ++s) {
+          const double x = UN[s];
+          if (x < 0.0) rem += (double)n.comp[nu * S + s] * x;
+        }
+        RW[nu] = rem;
+      }
+      for (int s = 0; s < S; ++s)
+        if (UN[s] < 0.0) { UN[s] = 0.0; st |= KR_DST_CLAMPED_NEG; any = true; }
+      for (int nu = 0; any && nu < E; ++nu) {
+        const double rem = RW[nu];
+        if (rem == 0.0) continue;
+        int res = -1;
+        double best = 0.0;
+        for (int s = 0; s < S; ++s) {
+          if (!n.resv[nu * S + s]) continue;
+          const double x = UN[s];
+          if (res < 0 || x > best) { res = s; best = x; }
+        }
+        if (res < 0) { st |= KR_DST_NO_RESERVOIR; continue; }
+        const double x = best + rem / (double)n.comp[nu * S + res];
+        UN[res] = x;
+        if (x < 0.0) st |= KR_DST_NEEDS_STAGE3;
+      }
+      if (a.status) a.status[cell] = st;
+    } else if (G.gl == 0 && a.status) {
+      a.status[cell] = st;
+    }
+    G.sync();
+    for (int s = G.gl; s < S; s += GT) a.y[cell * S + s] = UN[s];
+    if (ENERGY && G.gl == 0) a.T[cell] = UN[S];
+    G.sync();
+  }
+  if (G.gl == 0) {
+    atomicAdd(a.stats + 0, c_acc); atomicAdd(a.stats + 1, c_rej); atomicAdd(a.stats + 2, c_newton);
+    atomicAdd(a.stats + 3, c_newton); atomicAdd(a.stats + 4, c_rate); atomicAdd(a.stats + 5, c_failed);
+    if (c_ref) atomicAdd(a.stats + 6, c_ref);
+  }
+}

@@ -88,6 +88,17 @@ def test_specialised_kernel_compiles_for_sm100a_without_a_gpu(B, idx):
     assert "error" not in out["log"].lower()
 
 
+@pytest.mark.parametrize("idx,mode,warps", [(3, 0, 1), (3, 1, 1), (4, 0, 2), (4, 1, 1), (1, 1, 1)])
+def test_register_tile_kernel_compiles_for_sm100a_without_a_gpu(B, idx, mode, warps):
+    """csrc/kr_wpc.cuh (warp-per-cell, matrix in register tiles; fp64 and mixed precision) is compiled by NVRTC for
+    the sizes of the network at kr_network_create; the same compilation is checked here without a GPU.  The
+    static_assert inside the kernel ties the host's shared-memory layout to the device's."""
+    out = B.wpc_compile(w.make_network(idx), mode, warps)
+    assert out["cubin_bytes"] > 10000
+    assert "error" not in out["log"].lower()
+    assert "tiles" in out["log"]
+
+
 def test_null_and_nonsense_arguments(B):
     lib = B.load()
     assert lib.kr_network_create(None, None) == B.KR_EINVAL
