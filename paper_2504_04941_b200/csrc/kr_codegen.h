@@ -6,11 +6,16 @@
 #include <string>
 #include <vector>
 
+#include "kr_tables.h"
+
 struct KrHostNet {
   int E = 0, S = 0, R = 0, N = 0, energy = 0, n_aux = 0, any_rev = 0, any_tb = 0, any_qext = 0;
   double T_lo = 0, T_hi = 0, ln_p0_kB = 0;
   std::vector<int> sp, nu, flags, auxi, dnu_tot, comp, resv, row_ptr, col_ptr, row_ent, col_ent;
   std::vector<double> c0, A, beta, Ea, qk, tb, nasa, T_mid;
+  // programs of the register-tile kernel (empty when N > 64)
+  std::vector<KrDEnt> cprog, rprog;
+  std::vector<int> cprog_ptr, rprog_ptr, fac, tgt;
 };
 
 namespace kr_codegen {

@@ -327,7 +327,12 @@ kr_spec_kernel(const KrOptsDev o, const KrStepArgs g) {
         phase = (cell < g.n_cells) ? KRS_INIT : KRS_DONE;
       }
     }
+#ifdef KRS_SYNC
+    // all warps of the block walk the (long, fully unrolled) iteration body together: one instruction stream per SM
+    if (__syncthreads_and(phase == KRS_DONE)) break;
+#else
     if (__all_sync(0xffffffffu, phase == KRS_DONE)) break;
+#endif
 
     if (phase == KRS_INIT) {                                     // step 1
       st = 0;

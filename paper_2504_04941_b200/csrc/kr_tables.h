@@ -9,6 +9,16 @@
 #define KR_T_REF 300.0
 #define KR_EXP_CLAMP 690.0
 
+// One multiplicative term of the analytic Jacobian (eq. 19) as the register-tile kernel evaluates it:
+//   d = coef * D[g0] * D[g1] * D[g2] * D[g3],   D = the cell's shared-memory block viewed as doubles
+// (g0: k_f / k_r / qhat of reaction r; g1, g2: number densities of the remaining factors or the constant 1; g3: the
+// third-body factor M_r or 1).  d = dq_r / dn_m.  Built on the host (kr_lib.cu, build_programs).
+struct KrDEnt {
+  int g0, g1, g2, g3;
+  double coef;
+  int r, m;
+};
+
 struct KrNetDev {
   int E, S, R, N;        // conservation rows, species, reactions, unknowns (S or S+1)
   int energy;            // 1: T is the last unknown
@@ -41,6 +51,13 @@ struct KrNetDev {
   const int* row_ent;    // packed (reaction << 8) | (dnu + 128)
   const int* col_ptr;    // [S+1]  column list of species m
   const int* col_ent;    // packed (reaction << 4) | slot, slot 0..5 = participant slot, 15 = third-body only
+  // programs of the register-tile kernel (kr_wpc.cuh); null when N > 64
+  const KrDEnt* cprog;   // derivative terms grouped by column m: cprog_ptr[m] .. cprog_ptr[m+1]
+  const int* cprog_ptr;  // [S+1]
+  const KrDEnt* rprog;   // the same terms grouped by reaction r: rprog_ptr[r] .. rprog_ptr[r+1]
+  const int* rprog_ptr;  // [R+1]
+  const int* fac;        // [R*6] mass-action factors with powers expanded: 3 forward, 3 reverse species, S = the constant 1
+  const int* tgt;        // [R*8] [0] = number of rows the reaction feeds, then (row | (dnu + 128) << 8) with the net dnu
 };
 
 struct KrOptsDev {

@@ -21,7 +21,7 @@
 //                       rows as well (Gauss-Jordan form of Algorithm 1's elimination), which
 //                       removes the serial back substitution: after N columns row p_k holds x_k * pivot_k.
 //   mixed precision   : J is assembled in fp32, rows are scaled to unit max-norm, the elimination runs in fp32 and
-//                       its multipliers are kept (N^2 floats in the space J occupied); the linear residual
+//                       its column vectors are kept (N^2 floats in the space J occupied); the linear residual
 //                       r = -G - (I - hJ) d is formed in fp64 WITHOUT a stored fp64 matrix (J d is the analytic
 //                       directional derivative, one pass over the reactions) and the correction is obtained by
 //                       replaying the kept multipliers on r -- refinement until the correction is far below the
@@ -65,7 +65,8 @@ constexpr int oB = oF + 8 * N;                          // double[N]  -G
 constexpr int oX = oB + 8 * N;                          // double[N]  Newton update delta
 constexpr int oRS = oX + 8 * N;                         // double[N]  residual of the linear system (mixed)
 constexpr int oVI = oRS + 8 * N;                        // double[N]  1 / row scale
-constexpr int oTH = oVI + 8 * N;                        // double[3S] ghat, uhat, chat
+constexpr int oNN = oVI + 8 * N;                        // double[S+1] number densities n_s = Ncal y_s, then the constant 1
+constexpr int oTH = oNN + 8 * (S + 1);                  // double[3S] ghat, uhat, chat
 constexpr int oKF = oTH + 8 * 3 * S;                    // double[R]
 constexpr int oKR = oKF + 8 * R;                        // double[R]
 constexpr int oQ = oKR + 8 * R;                         // double[R]  q_r, later dq_r (mixed refinement)
@@ -79,11 +80,14 @@ constexpr int oLK = a8(oUR + int(sizeof(MT)) * NCG * CB);   // MT[2 LTS] multipl
 constexpr int oKOF = a8(oLK + int(sizeof(MT)) * 2 * LTS);   // int[TR RB] column in which row i was the pivot row
 constexpr int oPOF = a8(oKOF + 4 * TR * RB);            // int[N]     pivot row of column k
 constexpr int oPIV = a8(oPOF + 4 * N);                  // int[2]     pivot row of the current column (double buffered)
-constexpr int oMAT = a8(oPIV + 8);                      // MT[MAT_ELEMS]
+constexpr int oPVS = a8(oPIV + 8);                      // MT[2]      pivot value of the current column (double buffered)
+constexpr int oMAT = a8(oPVS + 2 * int(sizeof(MT)));    // MT[MAT_ELEMS]
 constexpr int CELL_BYTES = a8(oMAT + int(sizeof(MT)) * MAT_ELEMS);
 
 #ifdef KRW_CELL_BYTES
 static_assert(CELL_BYTES == KRW_CELL_BYTES, "host and device disagree on the shared-memory layout");
+static_assert(oNN == 8 * KRW_I_NN && oKF == 8 * KRW_I_KF && oKR == 8 * KRW_I_KR, "host and device disagree on the vector offsets");
+static_assert(!KRW_ANY_TB || (oQH == 8 * KRW_I_QH && oMT == 8 * KRW_I_MT), "host and device disagree on the third-body offsets");
 #endif
 
 struct Cell {
@@ -148,13 +152,6 @@ struct Grp {
   }
 };
 
-__device__ __forceinline__ double ipow(double x, int e) {          // e in 0..3 (R20)
-  double p = 1.0;
-  if (e >= 1) p = x;
-  if (e >= 2) p *= x;
-  if (e >= 3) p *= x;
-  return p;
-}
 __device__ __forceinline__ bool finite(double x) { return fabs(x) <= 1.79769313486231570e308; }
 __device__ __forceinline__ MT mt_rcp(MT x) {
 #if KRW_MIXED
@@ -179,17 +176,16 @@ __device__ __forceinline__ void thermo(const KrNetDev& n, const Cell& c, const G
 }
 
 // ---- steps 3-4: thread <-> reaction.  Rate constants (eq. 16 with R4, detailed balance R5, unary R16/R17) when
-// computeK, then q_r, dq_r/dT, and the third-body factors.  Returns partial sums of (q_ext/k_B) q and (q_ext/k_B) dq/dT.
-__device__ __forceinline__ void reactions(const KrNetDev& n, const Cell& c, const Grp& G, double Ncal, double invT, double lnT,
+// computeK, then q_r, dq_r/dT, and the third-body factors.  Number densities come from NN (filled by eval), the
+// mass-action products from the host-built factor lists (powers expanded, the constant 1 for unused factors).
+// Returns partial sums of (q_ext/k_B) q and (q_ext/k_B) dq/dT.
+__device__ __forceinline__ void reactions(const KrNetDev& n, const Cell& c, const Grp& G, double invT, double lnT,
                                           double aux0, const double* __restrict__ aux, long long cell, long long n_cells,
                                           bool computeK, double& heat_sum, double& heat_dT) {
-  double *U = c.d(oU), *TH = c.d(oTH), *KF = c.d(oKF), *KR = c.d(oKR), *Q = c.d(oQ);
+  double *NN = c.d(oNN), *TH = c.d(oTH), *KF = c.d(oKF), *KR = c.d(oKR), *Q = c.d(oQ);
   heat_sum = 0.0; heat_dT = 0.0;
   for (int r = G.gl; r < R; r += GT) {
     const int fl = n.flags[r];
-    int sp[6], nu[6];
-#pragma unroll
-    for (int k = 0; k < 6; ++k) { sp[k] = n.sp[6 * r + k]; nu[k] = n.nu[6 * r + k]; }
     double kf, kr = 0.0, dlf = 0.0, dlr = 0.0;
     if (computeK) {
       if (fl & KR_DF_CONST) kf = n.A[r];
@@ -203,13 +199,13 @@ __device__ __forceinline__ void reactions(const KrNetDev& n, const Cell& c, cons
         dlf = (beta + Ea * invT) * invT;
         if (fl & KR_DF_REV) {
           double sg = 0.0, su = 0.0;
-#pragma unroll
-          for (int k = 0; k < 6; ++k)
-            if (sp[k] >= 0) {
-              const double cf = (k < 3) ? -(double)nu[k] : (double)nu[k];
-              sg += cf * TH[sp[k]];
-              su += cf * TH[S + sp[k]];
-            }
+          const int nt = n.tgt[8 * r];
+          for (int t = 0; t < nt; ++t) {
+            const int e = n.tgt[8 * r + 1 + t];
+            const double cf = (double)((e >> 8) - 128);
+            sg += cf * TH[e & 255];
+            su += cf * TH[S + (e & 255)];
+          }
           const double lnKc = -sg + (double)n.dnu_tot[r] * (n.ln_p0_kB - lnT);
           kr = krs_exp(lnkf - lnKc);
           dlr = dlf - su * invT;
@@ -219,18 +215,14 @@ __device__ __forceinline__ void reactions(const KrNetDev& n, const Cell& c, cons
     } else {
       kf = KF[r]; kr = KR[r];
     }
-    double Pf = 1.0, Pr = 1.0;
-#pragma unroll
-    for (int k = 0; k < 6; ++k)
-      if (sp[k] >= 0) {
-        const double p = ipow(Ncal * U[sp[k]], nu[k]);
-        if (k < 3) Pf *= p; else Pr *= p;
-      }
+    const int* fc = n.fac + 6 * r;
+    const double Pf = NN[fc[0]] * NN[fc[1]] * NN[fc[2]];
+    const double Pr = NN[fc[3]] * NN[fc[4]] * NN[fc[5]];
     double Mtb = 1.0;
     const double qhat = kf * Pf - kr * Pr;
     if (KRW_ANY_TB && (fl & KR_DF_TB)) {
       Mtb = 0.0;
-      for (int s = 0; s < S; ++s) Mtb += n.tb_eff[r * S + s] * (Ncal * U[s]);
+      for (int s = 0; s < S; ++s) Mtb += n.tb_eff[r * S + s] * NN[s];
       c.d(oQH)[r] = qhat; c.d(oMT)[r] = Mtb;
     }
     const double q = Mtb * qhat;
@@ -264,41 +256,26 @@ __device__ __forceinline__ void rows(const KrNetDev& n, const Cell& c, const Grp
   }
 }
 
-// ---- Jacobian columns (eq. 19): thread <-> column m.  invC = 1 / sum_s y_s chat_s (energy equation only).
-__device__ __forceinline__ void columns(const KrNetDev& n, const Cell& c, const Grp& G, double Ncal, double T, double invC) {
-  double *U = c.d(oU), *TH = c.d(oTH), *KF = c.d(oKF), *KR = c.d(oKR);
+// ---- Jacobian columns (eq. 19): thread <-> column m, one host-built term d = dq_r/dn_m after the other, each scattered
+// to the rows its reaction feeds.  invC = 1 / sum_s y_s chat_s (energy equation only).
+__device__ __forceinline__ void columns(const KrNetDev& n, const Cell& c, const Grp& G, double T, double invC) {
+  const double* D = c.d(0);
+  double* TH = c.d(oTH);
   MT* J = c.m(oMAT);
   for (int m = G.gl; m < S; m += GT) {
     for (int i = 0; i < N; ++i) J[i * LD + m] = (MT)0;
     double heat_dn = 0.0;
-    const double nm = Ncal * U[m];
-    const int p1 = n.col_ptr[m + 1];
-    for (int p = n.col_ptr[m]; p < p1; ++p) {
-      const int ent = n.col_ent[p];
-      const int r = ent >> 4, slot = ent & 15;
-      int sp[6], nu[6];
-#pragma unroll
-      for (int k = 0; k < 6; ++k) { sp[k] = n.sp[6 * r + k]; nu[k] = n.nu[6 * r + k]; }
-      double d;
-      if (slot < 6) {
-        const int base = (slot < 3) ? 0 : 3;
-        double others = 1.0;
-        int e = 1;
-#pragma unroll
-        for (int k = 0; k < 6; ++k) {
-          if (k == slot) e = nu[k];
-          else if (k >= base && k < base + 3 && sp[k] >= 0) others *= ipow(Ncal * U[sp[k]], nu[k]);
-        }
-        const double kk2 = (slot < 3) ? KF[r] : -KR[r];
-        const double Mtb = (KRW_ANY_TB && (n.flags[r] & KR_DF_TB)) ? c.d(oMT)[r] : 1.0;
-        d = Mtb * (kk2 * (double)e * ipow(nm, e - 1) * others);
-      } else {
-        d = n.tb_eff[r * S + m] * c.d(oQH)[r];
+    const int p1 = n.cprog_ptr[m + 1];
+    for (int p = n.cprog_ptr[m]; p < p1; ++p) {
+      const KrDEnt t = n.cprog[p];
+      const double d = t.coef * D[t.g0] * D[t.g1] * D[t.g2] * D[t.g3];
+      const int* tg = n.tgt + 8 * t.r;
+      const int nt = tg[0];
+      for (int q = 0; q < nt; ++q) {
+        const int e = tg[1 + q];
+        J[(e & 255) * LD + m] += (MT)((double)((e >> 8) - 128) * d);
       }
-#pragma unroll
-      for (int k = 0; k < 6; ++k)
-        if (sp[k] >= 0) J[sp[k] * LD + m] += (MT)(((k < 3) ? -(double)nu[k] : (double)nu[k]) * d);
-      if (ENERGY && KRW_ANY_QEXT) heat_dn += n.qk[r] * d;
+      if (ENERGY && KRW_ANY_QEXT) heat_dn += n.qk[t.r] * d;
     }
     if (ENERGY) {
       double acc = 0.0;
@@ -311,13 +288,15 @@ __device__ __forceinline__ void columns(const KrNetDev& n, const Cell& c, const 
 // ---- full evaluation of f (and J) at U.  Thermo / KF / KR valid as the flags say.  Leaves 1/C and sum_s chat_s f_s
 // in the scalar slots (used by the matrix-free product of the mixed mode).
 __device__ __forceinline__ void eval(const KrNetDev& n, const Cell& c, const Grp& G, double Ncal, double T, double aux0,
-                                     const double* __restrict__ aux, long long cell, long long n_cells, bool computeK,
-                                     bool wantJ) {
+                                  const double* __restrict__ aux, long long cell, long long n_cells, bool computeK,
+                                  bool wantJ) {
   const double invT = krs_rcp(T), lnT = (ENERGY || computeK) ? log(T) : 0.0;
   const double invN = krs_rcp(Ncal);
-  double *U = c.d(oU), *TH = c.d(oTH), *F = c.d(oF);
+  double *U = c.d(oU), *TH = c.d(oTH), *F = c.d(oF), *NN = c.d(oNN);
+  for (int s = G.gl; s <= S; s += GT) NN[s] = (s < S) ? Ncal * U[s] : 1.0;
+  G.sync();
   double red[3];
-  reactions(n, c, G, Ncal, invT, lnT, aux0, aux, cell, n_cells, computeK, red[0], red[1]);
+  reactions(n, c, G, invT, lnT, aux0, aux, cell, n_cells, computeK, red[0], red[1]);
   red[2] = 0.0;
   if (ENERGY) {
     for (int s = G.gl; s < S; s += GT) red[2] += U[s] * TH[2 * S + s];
@@ -327,7 +306,7 @@ __device__ __forceinline__ void eval(const KrNetDev& n, const Cell& c, const Grp
   const double heat_sum = red[0], heat_dT = red[1];
   const double invC = ENERGY ? krs_rcp(red[2]) : 1.0;
   rows(n, c, G, invN, wantJ);
-  if (wantJ) columns(n, c, G, Ncal, T, invC);
+  if (wantJ) columns(n, c, G, T, invC);
   G.sync();
   if (ENERGY) {
     MT* J = c.m(oMAT);
@@ -351,41 +330,21 @@ __device__ __forceinline__ void eval(const KrNetDev& n, const Cell& c, const Grp
 #if KRW_MIXED
 // ---- mixed mode: RS = B - (I - hJ) X in fp64 without a stored fp64 matrix.  J X is the analytic directional
 // derivative of f along X with exactly the terms of DESIGN.md step 5: per reaction
-//   dq_r = M_r sum_slots (k e n^(e-1) prod others) dn_slot + (third body) qhat_r sum_s eff_s dn_s + (dq_r/dT) dT,
+//   dq_r = sum_terms (dq_r/dn_m) Ncal X_m  (the terms of the Jacobian program, grouped by reaction) + (dq_r/dT) X_T,
 // then (J X)_s = (1/Ncal) sum_r dnu_rs dq_r and (J X)_T = [ (1/Ncal) sum_r (q_ext/k_B) dq_r - T sum_s uhat_s (J X)_s
-// - (sum_s chat_s f_s) dT ] / C.
+// - (sum_s chat_s f_s) X_T ] / C.
 __device__ __forceinline__ void residual(const KrNetDev& n, const Cell& c, const Grp& G, double Ncal, double T, double h) {
-  double *U = c.d(oU), *TH = c.d(oTH), *KF = c.d(oKF), *KR = c.d(oKR), *DQ = c.d(oQ), *X = c.d(oX), *B = c.d(oB),
-         *RS = c.d(oRS);
+  const double* D = c.d(0);
+  double *TH = c.d(oTH), *DQ = c.d(oQ), *X = c.d(oX), *B = c.d(oB), *RS = c.d(oRS);
   const double invN = krs_rcp(Ncal);
   const double dT = ENERGY ? X[S] : 0.0;
   double red[2] = {0.0, 0.0};
   for (int r = G.gl; r < R; r += GT) {
-    int sp[6], nu[6];
-#pragma unroll
-    for (int k = 0; k < 6; ++k) { sp[k] = n.sp[6 * r + k]; nu[k] = n.nu[6 * r + k]; }
-    const int fl = n.flags[r];
-    const double kf = KF[r], kr = KR[r];
-    double nn[6];
-#pragma unroll
-    for (int k = 0; k < 6; ++k) nn[k] = (sp[k] >= 0) ? Ncal * U[sp[k]] : 1.0;
     double dq = 0.0;
-#pragma unroll
-    for (int k = 0; k < 6; ++k) {
-      if (sp[k] < 0) continue;
-      if (k >= 3 && !(fl & KR_DF_REV)) continue;
-      const int base = (k < 3) ? 0 : 3;
-      double others = 1.0;
-#pragma unroll
-      for (int kk = 0; kk < 3; ++kk)
-        if (base + kk != k && sp[base + kk] >= 0) others *= ipow(nn[base + kk], nu[base + kk]);
-      const double kk2 = (k < 3) ? kf : -kr;
-      dq += kk2 * (double)nu[k] * ipow(nn[k], nu[k] - 1) * others * (Ncal * X[sp[k]]);
-    }
-    if (KRW_ANY_TB && (fl & KR_DF_TB)) {
-      double dM = 0.0;
-      for (int s = 0; s < S; ++s) dM += n.tb_eff[r * S + s] * (Ncal * X[s]);
-      dq = c.d(oMT)[r] * dq + c.d(oQH)[r] * dM;
+    const int p1 = n.rprog_ptr[r + 1];
+    for (int p = n.rprog_ptr[r]; p < p1; ++p) {
+      const KrDEnt t = n.rprog[p];
+      dq += t.coef * D[t.g0] * D[t.g1] * D[t.g2] * D[t.g3] * (Ncal * X[t.m]);
     }
     if (ENERGY) dq += c.d(oDQT)[r] * dT;
     DQ[r] = dq;
@@ -421,20 +380,32 @@ struct Lane {
   __device__ __forceinline__ explicit Lane(int gl) : lane(gl & 31), wq(gl >> 5), tr((gl & 31) / TC), tc((gl & 31) % TC),
                                                      cg((gl >> 5) * TC + (gl & 31) % TC) {}
 };
-__device__ __forceinline__ int lidx(int row) { return row + row / RB; }     // padded index into a multiplier vector
+__device__ __forceinline__ int lidx(int row) { return row + row / RB; }     // padded index into a column vector
 
 template <int I>
-__device__ __forceinline__ void publish_row(const MT (&a)[RB][CB], int kb, MT* UR, int cg) {
+__device__ __forceinline__ void publish_row(const MT (&a)[RB][CB], MT (&sc)[RB], int kb, MT* UR, int cg) {
 #pragma unroll
   for (int j = 0; j < CB; ++j)
     if (j >= kb) UR[j * NCG + cg] = a[I][j];
+  sc[I] = (MT)-1;                            // the row is used: never a pivot candidate again
 }
 
 #define KRW_PUB_CASE(I) \
-  case I: if constexpr (I < RB) publish_row<(I < RB ? I : 0)>(a, kb, UR, L.cg); break;
+  case I: if constexpr (I < RB) publish_row<(I < RB ? I : 0)>(a, sc, kb, UR, L.cg); break;
+
+// pivot key of a candidate: the leading bits of |a| / scale with the row index in the 6 low bits, so that ONE integer
+// maximum gives the scaled pivot of Algorithm 1 and the tie rule (smallest row).  Candidates closer than 2^-46
+// (fp64, 64-bit key) / 2^-17 (fp32, 32-bit key) relative count as tied; used rows carry a negative scale and lose.
+#if KRW_MIXED
+typedef int KeyT;
+__device__ __forceinline__ KeyT pivot_key(MT t, int row) { return (__float_as_int(t) | 63) - row; }
+#else
+typedef long long KeyT;
+__device__ __forceinline__ KeyT pivot_key(MT t, int row) { return (__double_as_longlong(t) | 63LL) - (long long)row; }
+#endif
 
 // Pass A (thread <-> row): B = -(U - UN - h F), row scales of I - hJ.  Pass B: tiles.  Then N elimination columns.
-// On success X holds the solution of (I - hJ) X = B; in mixed mode the multipliers, reciprocal pivots and the row
+// On success X holds the solution of (I - hJ) X = B; in mixed mode the column vectors, reciprocal pivots and the row
 // order stay in shared memory for replay().  Uniform return value (false: zero row, non-finite entry or no pivot).
 __device__ __forceinline__ bool eliminate(const Cell& c, const Grp& G, double h) {
   const Lane L(G.gl);
@@ -445,13 +416,14 @@ __device__ __forceinline__ bool eliminate(const Cell& c, const Grp& G, double h)
   for (int i = G.gl; i < N; i += GT) {
     B[i] = -(U[i] - UN[i] - h * F[i]);
     MT big = (MT)0;
+    bool fin = true;
     for (int j = 0; j < N; ++j) {
       const MT x = ((i == j) ? (MT)1 : (MT)0) - hm * J[i * LD + j];
       const MT ax = fabs(x);
       big = (ax > big) ? ax : big;
-      if (!(ax <= (MT)(MIXED ? 3.0e38 : 1.7e308))) big = ax;      // keep inf / NaN: the row is refused below
+      fin = fin && (ax <= (MT)(MIXED ? 3.0e38 : 1.7e308));        // false for inf and NaN
     }
-    const bool ok = (big > (MT)(MIXED ? 1e-30 : 1e-300)) && (big <= (MT)(MIXED ? 3.0e38 : 1.7e308));
+    const bool ok = fin && (big > (MT)(MIXED ? 1e-30 : 1e-300));
     rows_ok = rows_ok && ok;
     VI[i] = ok ? 1.0 / (double)big : 0.0;
   }
@@ -460,19 +432,13 @@ __device__ __forceinline__ bool eliminate(const Cell& c, const Grp& G, double h)
   if (!rows_ok) return false;
 
   MT a[RB][CB];
-#if !KRW_MIXED
-  double vinv[RB];
-#endif
-  unsigned alive = 0;
+  MT sc[RB];                                  // > 0: 1 / row scale of a candidate row;  < 0: used or padding row
 #pragma unroll
   for (int i = 0; i < RB; ++i) {
     const int row = L.tr * RB + i;
     const bool rin = row < N;
     const double vi = rin ? VI[row] : 0.0;
-#if !KRW_MIXED
-    vinv[i] = vi;
-#endif
-    if (rin) alive |= 1u << i;
+    sc[i] = rin ? (MIXED ? (MT)1 : (MT)vi) : (MT)-1;
 #pragma unroll
     for (int j = 0; j < CB; ++j) {
       const int col = j * NCG + L.cg;
@@ -490,46 +456,43 @@ __device__ __forceinline__ bool eliminate(const Cell& c, const Grp& G, double h)
 
   MT* UR = c.m(oUR);
   MT* RP = c.m(oRP);
+  MT* PVS = c.m(oPVS);
   int* PIV = c.i(oPIV);
   int* KOF = c.i(oKOF);
+  int* POF = c.i(oPOF);
 #pragma unroll
   for (int kb = 0; kb < CB; ++kb) {
     for (int kc = 0; kc < NCG; ++kc) {
       const int k = kb * NCG + kc;
       if (k >= N) break;
       MT* Lk = MIXED ? (c.m(oMAT) + k * LTS) : (c.m(oLK) + (k & 1) * LTS);
-      if (W == 1 || L.wq == kc / TC) {        // the warp that holds column k: scaled pivot search (Algorithm 1)
-        MT best = (MT)-1, pv = (MT)0;
-        int bi = -1;
+      int p;
+      if (W == 1 || L.wq == kc / TC) {        // the warp that holds column k
+        const bool mine = (L.tc == kc % TC);
+        KeyT key = (KeyT)-1 << (8 * sizeof(KeyT) - 2);
 #pragma unroll
         for (int i = 0; i < RB; ++i) {
-#if KRW_MIXED
-          const MT t = fabsf(a[i][kb]);
-#else
-          const MT t = fabs(a[i][kb]) * vinv[i];
-#endif
-          if (((alive >> i) & 1u) && t > best) { best = t; pv = a[i][kb]; bi = L.tr * RB + i; }
+          const MT v = a[i][kb];
+          if (mine) Lk[L.tr * RB + i + L.tr] = v;                  // column k as it stands (the multipliers x pivot)
+          const KeyT ki = pivot_key(fabs(v) * sc[i], L.tr * RB + i);
+          key = (ki > key) ? ki : key;
         }
 #pragma unroll
         for (int off = TC; off < 32; off <<= 1) {
-          const MT t2 = __shfl_xor_sync(0xffffffffu, best, off);
-          const MT p2 = __shfl_xor_sync(0xffffffffu, pv, off);
-          const int i2 = __shfl_xor_sync(0xffffffffu, bi, off);
-          if (i2 >= 0 && (bi < 0 || t2 > best || (t2 == best && i2 < bi))) { best = t2; pv = p2; bi = i2; }
+          const KeyT k2 = __shfl_xor_sync(0xffffffffu, key, off);
+          key = (k2 > key) ? k2 : key;
         }
-        if (L.tc == kc % TC) {
-          const bool okp = (bi >= 0) && (fabs(pv) >= (MT)(MIXED ? 1e-30 : 1e-300));
-          const MT rp = mt_rcp(okp ? pv : (MT)1);
-#pragma unroll
-          for (int i = 0; i < RB; ++i) {
-            const int row = L.tr * RB + i;
-            Lk[row + L.tr] = (row == bi) ? (MT)0 : a[i][kb] * rp;
-          }
-          if (L.tr == 0) { PIV[k & 1] = okp ? bi : -1; RP[k] = rp; }
+        key = __shfl_sync(0xffffffffu, key, kc % TC);              // lane (tr 0, tc of column k) holds the column's maximum
+        p = (key >= 0) ? (63 - (int)(key & 63)) : -1;
+        if (mine && p >= 0 && p / RB == L.tr) {                     // the lane that holds a[p][k]
+          const int ix = p + L.tr;
+          PVS[k & 1] = Lk[ix];
+          Lk[ix] = (MT)0;                                            // row p itself is not updated
+          if (W > 1) PIV[k & 1] = p;
         }
+        if (W > 1 && p < 0 && L.lane == 0) PIV[k & 1] = -1;
       }
-      G.sync();
-      const int p = PIV[k & 1];
+      if (W > 1) { G.sync(); p = PIV[k & 1]; }
       if (p < 0) return false;
       const int trp = p / RB, ip = p - trp * RB;
       if (L.tr == trp) {                      // the lanes that hold row p publish it and retire it
@@ -540,13 +503,16 @@ __device__ __forceinline__ bool eliminate(const Cell& c, const Grp& G, double h)
           KRW_PUB_CASE(19) KRW_PUB_CASE(20) KRW_PUB_CASE(21)
           default: break;
         }
-        alive &= ~(1u << ip);
-        if (L.cg == 0) { KOF[p] = k; c.i(oPOF)[k] = p; }
+        if (L.cg == 0) { KOF[p] = k; POF[k] = p; }
       }
       __syncwarp();
+      const MT pv = PVS[k & 1];
+      if (!(fabs(pv) >= (MT)(MIXED ? 1e-30 : 1e-300)) || !(fabs(pv) <= (MT)(MIXED ? 3.0e38 : 1.7e308))) return false;
+      const MT rp = mt_rcp(pv);
+      if (L.cg == 0 && L.tr == 0) RP[k] = rp;
       MT l[RB], u[CB];
 #pragma unroll
-      for (int i = 0; i < RB; ++i) l[i] = Lk[L.tr * RB + i + L.tr];
+      for (int i = 0; i < RB; ++i) l[i] = Lk[L.tr * RB + i + L.tr] * rp;
 #pragma unroll
       for (int j = 0; j < CB; ++j)
         if (j >= kb) u[j] = UR[j * NCG + L.cg];
@@ -595,11 +561,11 @@ __device__ __forceinline__ void replay(const Cell& c, const Grp& G, const KrOpts
     float mine = r[0];
 #pragma unroll
     for (int q = 1; q < NRL; ++q) mine = ((p >> 5) == q) ? r[q] : mine;
-    const float rp = __shfl_sync(0xffffffffu, mine, p & 31);
+    const float rp = __shfl_sync(0xffffffffu, mine, p & 31) * RP[k];   // r_p / pivot_k
 #pragma unroll
     for (int q = 0; q < NRL; ++q) {
       const int row = lane + 32 * q;
-      if (row < N) r[q] = fmaf(-LT[k * LTS + lidx(row)], rp, r[q]);
+      if (row < N) r[q] = fmaf(-LT[k * LTS + lidx(row)], rp, r[q]);       // column k (zero at row p) times r_p / pivot_k
     }
   }
   double xn[NRL];
@@ -680,11 +646,8 @@ kr_wpc_kernel(const KrNetDev n, const KrOptsDev o, const KrStepArgs a) {
       const double invT = krs_rcp(Tc), lnT = log(Tc);
       if (!ENERGY) {
         if (KRW_ANY_REV) { thermo(n, c, G, Tc, invT, lnT); G.sync(); }
-        if (o.h0_mode != 1) {          // rate constants only (the h0 evaluation below computes them as well)
-          double hs, hd;
-          reactions(n, c, G, Ncal, invT, lnT, aux0, a.aux, cell, a.n_cells, true, hs, hd);
-          G.sync();
-        }
+        if (o.h0_mode != 1)            // rate constants (the h0 evaluation below computes them as well)
+          eval(n, c, G, Ncal, Tc, aux0, a.aux, cell, a.n_cells, true, false);
         c_rate++;
       }
       if (o.h0_mode == 1) {
