@@ -13,7 +13,9 @@
 //                   compile-time select chains (no dynamic register index), U stored back to shared memory,
 //                   right-hand side carried along, back substitution                  (Algorithm 1, R14)
 // Persistent kernel: one Newton iteration is the unit of lock-step; finished lanes refill from the global
-// work counter (a8).
+// work counter (a8).  The unrolled iteration body is ~10^4 instructions, far beyond the instruction caches, so the
+// kernel runs ONE block of 8 warps per SM that walks the body in lock-step (block barriers, no divergent code in
+// the body): every instruction fetched from L2 serves all resident warps.
 #pragma once
 #include "kr_tables.h"
 #include "kr_math.cuh"
@@ -238,9 +240,8 @@ __device__ __forceinline__ bool krs_lu_solve(const KrsShared& sh, const int (&vh
   KR_FOR(i, 0, N)
     perm[i] = i;
     ok = ok && (vh[i] >= 0x00100000) && (vh[i] < 0x7ff00000);      // zero / denormal / non-finite row
-    v[i] = krs_rcp(__hiloint2double(vh[i], 0));
+    v[i] = krs_rcp(__hiloint2double(ok ? vh[i] : 0x3ff00000, 0));
   KR_END
-  if (!ok) return false;
   KR_FOR(j, 0, N)
     double c[N];
     KR_FOR(i, 0, N) c[i] = sh.M(perm[i], j); KR_END
@@ -281,18 +282,28 @@ __device__ __forceinline__ bool krs_lu_solve(const KrsShared& sh, const int (&vh
     KR_FOR(i, 0, j) sh.M(i, j) = c[i]; KR_END              // U(0..j-1, j): column j of shared memory is free now
     sh.M(j, j) = rp;                                       // the reciprocal pivot, for the back substitution
   KR_END
-  if (!ok) return false;
   KR_FOR(ii, 0, N)
     constexpr int i = N - 1 - ii;
     double sum = rhs[i];
     KR_FOR(k, i + 1, N) sum -= sh.M(i, k) * rhs[k]; KR_END
     rhs[i] = sum * sh.M(i, i);
   KR_END
-  return true;
+  return ok;                                               // no early exit: every lane of the block walks the same code
 }
 
-enum { KRS_FETCH = 0, KRS_INIT = 1, KRS_NEWTON = 2, KRS_DONE = 3 };
+enum { KRS_FETCH = 0, KRS_RUN = 1, KRS_DONE = 2 };
 
+#ifdef KRS_SYNC
+#define KRS_ALIGN() __syncthreads()      // keeps the 8 warps of the block on one instruction stream inside the body too
+#else
+#define KRS_ALIGN() ((void)0)
+#endif
+
+// One trip of the main loop = one pass of EVERY lane through the same straight-line body: rate constants, reactions,
+// Jacobian columns, LU, update, controller.  A lane that has just loaded a cell uses its first pass as the
+// preliminary evaluation (rate constants of an isothermal cell, f(u_in) for the first sub-step, DESIGN.md step 1) and
+// discards the rest of that pass; idle lanes (no cells left) run the body on dead data.  Nothing in the body
+// diverges, so block-wide barriers inside it are legal and every warp of the block fetches the same instructions.
 extern "C" __global__ void __launch_bounds__(KRS_BLOCK, KRS_MIN_BLOCKS)
 kr_spec_kernel(const KrOptsDev o, const KrStepArgs g) {
   extern __shared__ double kr_sm[];
@@ -306,213 +317,219 @@ kr_spec_kernel(const KrOptsDev o, const KrStepArgs g) {
   long long cell = -1;
   double u[N];
   double kfi[R], kri[R];                       // isothermal networks: rate constants of the cell (registers)
-  double Ncal = 1.0, T_iso = 0.0, aux0 = 0.0, t = 0.0, h = 0.0, h_floor = 0.0, e = 0.0, e_prev = 0.0;
+  double Ncal = 1.0, T_iso = 1.0, aux0 = 0.0, t = 0.0, h = 1.0, h_floor = 0.0, e = 0.0, e_prev = 0.0;
   int k = 0, it = 0, st = 0, n_acc = 0, n_rej = 0;
-  bool last = false;
+  bool last = false, pend = false;
   unsigned long long c_acc = 0, c_rej = 0, c_newton = 0, c_rate = 0, c_failed = 0;
-  KR_FOR(i, 0, N) u[i] = 0.0; KR_END
+  KR_FOR(i, 0, N) u[i] = 1.0; sh.UN(i) = 1.0; KR_END
   KR_FOR(r, 0, R) kfi[r] = 0.0; kri[r] = 0.0; KR_END
 
   for (;;) {
     __syncwarp();
     const bool need = (phase == KRS_FETCH);
     const unsigned want = __ballot_sync(0xffffffffu, need);
-    if (want) {
+    if (want) {                                                  // step 1: a8 refill + layout-in
       const int leader = __ffs(want) - 1;
       unsigned long long base = 0;
       if (lane == leader) base = atomicAdd(g.counter, (unsigned long long)__popc(want));
       base = __shfl_sync(0xffffffffu, base, leader);
       if (need) {
         cell = (long long)(base + (unsigned long long)__popc(want & ((1u << lane) - 1u)));
-        phase = (cell < g.n_cells) ? KRS_INIT : KRS_DONE;
+        phase = (cell < g.n_cells) ? KRS_RUN : KRS_DONE;
+        if (phase == KRS_RUN) {
+          st = 0;
+          double Tc = g.T[cell];
+          constexpr double T_lo = KrNet::T_lo, T_hi = KrNet::T_hi;
+          if (Tc < T_lo) { Tc = T_lo; st |= KR_DST_T_CLAMPED; }
+          if (Tc > T_hi) { Tc = T_hi; st |= KR_DST_T_CLAMPED; }
+          Ncal = g.rho[cell] * (1.0 / KR_M_U);
+          KR_FOR(s, 0, S) u[s] = g.y[cell * S + s]; sh.UN(s) = u[s]; KR_END
+          if constexpr (KrNet::energy) { u[S] = Tc; sh.UN(S) = Tc; }
+          T_iso = Tc;
+          aux0 = (KrNet::n_aux > 0) ? g.aux[cell] : 0.0;
+          t = 0.0; h = g.dt; n_acc = 0; n_rej = 0; k = 0;
+          h_floor = o.h_min_rel * g.dt;
+          pend = (o.h0_mode == 1) || !KrNet::energy;
+        }
       }
     }
 #ifdef KRS_SYNC
-    // all warps of the block walk the (long, fully unrolled) iteration body together: one instruction stream per SM
     if (__syncthreads_and(phase == KRS_DONE)) break;
 #else
     if (__all_sync(0xffffffffu, phase == KRS_DONE)) break;
 #endif
+    const bool active = (phase == KRS_RUN);
+    const bool prelim = pend;                                    // this pass only evaluates (see above)
 
-    if (phase == KRS_INIT) {                                     // step 1
-      st = 0;
-      double Tc = g.T[cell];
-      constexpr double T_lo = KrNet::T_lo, T_hi = KrNet::T_hi;
-      if (Tc < T_lo) { Tc = T_lo; st |= KR_DST_T_CLAMPED; }
-      if (Tc > T_hi) { Tc = T_hi; st |= KR_DST_T_CLAMPED; }
-      Ncal = g.rho[cell] * (1.0 / KR_M_U);
-      KR_FOR(s, 0, S) u[s] = g.y[cell * S + s]; sh.UN(s) = u[s]; KR_END
-      if constexpr (KrNet::energy) { u[S] = Tc; sh.UN(S) = Tc; }
-      T_iso = Tc;
-      aux0 = (KrNet::n_aux > 0) ? g.aux[cell] : 0.0;
-      t = 0.0; h = g.dt; n_acc = 0; n_rej = 0;
-      double uh[S], ch[S], dlf[R], dlr[R];
-      if constexpr (!KrNet::energy) {
-        krs_rate_constants<false>(Tc, aux0, g.aux, cell, g.n_cells, kfi, kri, dlf, dlr, uh, ch);
-        c_rate++;
+    bool fail_cell = false, cell_done = false;
+    if (active && !prelim && k == 0) {                           // sub-step start: trim (R22), failure test
+      const double rem = g.dt - t;
+      last = false;
+      if (h >= rem) { h = rem; last = true; }
+      if (h < h_floor || n_acc + n_rej > o.max_substeps) fail_cell = true;
+      else {
+        KR_FOR(i, 0, N) u[i] = sh.UN(i); KR_END
+        e_prev = 0.0; e = __longlong_as_double(0x7ff0000000000000LL); it = K + 1; k = 1;
       }
-      if (o.h0_mode == 1) {
-        double n[S], f[N], a[R], b[R], qh[R], jt[N], Cv = 1.0, sc = 0.0;
-        if constexpr (KrNet::energy) {
-          double kf[R], kr[R];
-          krs_rate_constants<false>(Tc, aux0, g.aux, cell, g.n_cells, kf, kr, dlf, dlr, uh, ch);
-          c_rate++;
-          krs_reactions<false>(Ncal, Tc, u, kf, kr, dlf, dlr, uh, ch, n, f, a, b, qh, jt, Cv, sc);
-        } else {
-          krs_reactions<false>(Ncal, Tc, u, kfi, kri, dlf, dlr, uh, ch, n, f, a, b, qh, jt, Cv, sc);
-        }
-        double big = 0.0;
-        KR_FOR(s, 0, S) big = fmax(big, fabs(f[s]) / (fabs(u[s]) + o.y_floor)); KR_END
-        if (big > 0.0 && krs_finite(big)) h = fmin(g.dt, o.eta / big);
-      }
-      h_floor = o.h_min_rel * fmin(h, g.dt);
-      k = 0;
-      phase = KRS_NEWTON;
     }
-    __syncwarp();
+    const bool live = active && !prelim && !fail_cell;           // this pass is a Newton iteration of the lane's cell
 
-    if (phase == KRS_NEWTON) {
-      bool fail_cell = false, cell_done = false;
-      if (k == 0) {                                              // sub-step start: trim (R22), failure test
-        const double rem = g.dt - t;
-        last = false;
-        if (h >= rem) { h = rem; last = true; }
-        if (h < h_floor || n_acc + n_rej > o.max_substeps) fail_cell = true;
-        else {
-          KR_FOR(i, 0, N) u[i] = sh.UN(i); KR_END
-          e_prev = 0.0; e = __longlong_as_double(0x7ff0000000000000LL); it = K + 1; k = 1;
-        }
-      }
-      if (!fail_cell) {                                          // one Newton iteration (step 6)
-        const double T = KrNet::energy ? u[N - 1] : T_iso;
-        double rhs[N];
-        int vh[N];
-        {
-          double uh[S], ch[S], n[S], f[N], a[R], b[R], qh[R], jt[N], Cv = 1.0, sc = 0.0;
-          if constexpr (KrNet::energy) {
-            double kf[R], kr[R], dlf[R], dlr[R];
-            krs_rate_constants<true>(T, aux0, g.aux, cell, g.n_cells, kf, kr, dlf, dlr, uh, ch);
+    // ---- steps 2-5 ------------------------------------------------------------------------------------------
+    const double T = KrNet::energy ? u[N - 1] : T_iso;
+    double rhs[N];
+    int vh[N];
+    {
+      double uh[S], ch[S], n[S], f[N], a[R], b[R], qh[R], jt[N], Cv = 1.0, sc = 0.0;
+      if constexpr (KrNet::energy) {
+        double kf[R], kr[R], dlf[R], dlr[R];
+        krs_rate_constants<true>(T, aux0, g.aux, active ? cell : 0, g.n_cells, kf, kr, dlf, dlr, uh, ch);
+        if (active && !fail_cell) c_rate++;
+        KRS_ALIGN();
+        krs_reactions<true>(Ncal, T, u, kf, kr, dlf, dlr, uh, ch, n, f, a, b, qh, jt, Cv, sc);
+      } else {
+        double dlf[R], dlr[R];
+        if (__any_sync(0xffffffffu, active && prelim)) {         // rate constants of freshly loaded isothermal cells
+          double kf[R], kr[R];
+          krs_rate_constants<false>(T, aux0, g.aux, active ? cell : 0, g.n_cells, kf, kr, dlf, dlr, uh, ch);
+          if (active && prelim) {
+            KR_FOR(r, 0, R) kfi[r] = kf[r]; kri[r] = kr[r]; KR_END
             c_rate++;
-            krs_reactions<true>(Ncal, T, u, kf, kr, dlf, dlr, uh, ch, n, f, a, b, qh, jt, Cv, sc);
-          } else {
-            double dlf[R], dlr[R];
-            krs_reactions<true>(Ncal, T, u, kfi, kri, dlf, dlr, uh, ch, n, f, a, b, qh, jt, Cv, sc);
           }
-          KR_FOR(i, 0, N) vh[i] = 0; KR_END
-          KR_FOR(m, 0, S) krs_column<m>(sh, h, T, Cv, n, a, b, qh, uh, vh); KR_END
-          if constexpr (KrNet::energy) {                         // T column (eq. 20)
-            KR_FOR(i, 0, N)
-              const double x = ((i == S) ? 1.0 : 0.0) - h * jt[i];
-              sh.M(i, S) = x;
-              vh[i] = max(vh[i], __double2hiint(x) & 0x7fffffff);
-            KR_END
-          }
-          KR_FOR(i, 0, N) rhs[i] = -(u[i] - sh.UN(i) - h * f[i]); KR_END
         }
-        c_newton++;
-        bool ran = true, sub_end = false;
-        if (!krs_lu_solve(sh, vh, rhs)) { ran = false; sub_end = true; }
+        KRS_ALIGN();
+        krs_reactions<true>(Ncal, T, u, kfi, kri, dlf, dlr, uh, ch, n, f, a, b, qh, jt, Cv, sc);
+      }
+      if (active && prelim) {                                    // first sub-step from f(u_in) (step 1, h0_mode 1)
+        if (o.h0_mode == 1) {
+          double big = 0.0;
+          KR_FOR(s, 0, S) big = fmax(big, fabs(f[s]) / (fabs(u[s]) + o.y_floor)); KR_END
+          if (big > 0.0 && krs_finite(big)) h = fmin(g.dt, o.eta / big);
+        }
+        h_floor = o.h_min_rel * fmin(h, g.dt);
+        pend = false;
+      }
+      KRS_ALIGN();
+      KR_FOR(i, 0, N) vh[i] = 0; KR_END
+      KR_FOR(m, 0, S) krs_column<m>(sh, h, T, Cv, n, a, b, qh, uh, vh); KR_END
+      if constexpr (KrNet::energy) {                             // T column (eq. 20)
+        KR_FOR(i, 0, N)
+          const double x = ((i == S) ? 1.0 : 0.0) - h * jt[i];
+          sh.M(i, S) = x;
+          vh[i] = max(vh[i], __double2hiint(x) & 0x7fffffff);
+        KR_END
+      }
+      KR_FOR(i, 0, N) rhs[i] = -(u[i] - sh.UN(i) - h * f[i]); KR_END
+    }
+    KRS_ALIGN();
+    const bool solved = krs_lu_solve(sh, vh, rhs);               // step 7 (no early exits inside)
+    KRS_ALIGN();
+
+    if (live) {                                                  // steps 6-8 for the lanes this pass counts for
+      c_newton++;
+      bool ran = true, sub_end = false;
+      if (!solved) { ran = false; sub_end = true; }
+      else {
+        bool fin = true;
+        double en = 0.0;
+        KR_FOR(i, 0, N)
+          u[i] += rhs[i];
+          fin = fin && krs_finite(u[i]);
+          const double w = fabs(rhs[i]) * krs_rcp(o.rtol * fabs(u[i]) + ((i < S) ? o.atol_y : o.atol_T));
+          en = (w > en) ? w : en;
+        KR_END
+        if (!fin) { ran = false; sub_end = true; }
         else {
-          bool fin = true;
-          double en = 0.0;
+          e = en;
+          if (it == K + 1 && e <= 1.0) it = k;
+          if (!o.fixed_newton) {
+            if (e <= 1.0) sub_end = true;
+            else if (k >= 2 && e > o.bail_ratio * e_prev) { ran = false; sub_end = true; }
+          }
+          e_prev = e;
+          if (k >= K) sub_end = true;
+          k++;
+        }
+      }
+      if (sub_end) {                                             // step 8: accept / reject
+        bool ok = ran && (e <= 1.0);
+        if (ok) {
+          double miny = u[0];
+          KR_FOR(s, 1, S) miny = fmin(miny, u[s]); KR_END
+          if (!(miny >= -o.neg_tol)) ok = false;
+        }
+        if constexpr (KrNet::energy) {
+          constexpr double T_lo = KrNet::T_lo, T_hi = KrNet::T_hi;
+          if (ok && !(u[N - 1] >= T_lo && u[N - 1] <= T_hi)) ok = false;
+        }
+        if (ok && krs_finite(o.chg_max)) {
+          double chg = 0.0;
           KR_FOR(i, 0, N)
-            u[i] += rhs[i];
-            fin = fin && krs_finite(u[i]);
-            const double w = fabs(rhs[i]) * krs_rcp(o.rtol * fabs(u[i]) + ((i < S) ? o.atol_y : o.atol_T));
-            en = (w > en) ? w : en;
+            const double un = sh.UN(i);
+            chg = fmax(chg, fabs(u[i] - un) / ((i < S) ? (fabs(un) + o.chg_floor) : un));
           KR_END
-          if (!fin) { ran = false; sub_end = true; }
+          if (!(chg <= o.chg_max)) ok = false;
+        }
+        if (ok) {
+          n_acc++;
+          KR_FOR(i, 0, N) sh.UN(i) = u[i]; KR_END
+          if (last) cell_done = true;
           else {
-            e = en;
-            if (it == K + 1 && e <= 1.0) it = k;
-            if (!o.fixed_newton) {
-              if (e <= 1.0) sub_end = true;
-              else if (k >= 2 && e > o.bail_ratio * e_prev) { ran = false; sub_end = true; }
-            }
-            e_prev = e;
-            if (k >= K) sub_end = true;
-            k++;
+            t = t + h;
+            if (it <= o.it_fast) h = h * o.grow_fast;
+            else if (it <= o.it_mid) h = h * o.grow_mid;
           }
+        } else {
+          n_rej++;
+          st |= KR_DST_REJECTED;
+          h = h * o.shrink;
+          KR_FOR(i, 0, N) u[i] = sh.UN(i); KR_END               // keep the lane's state finite
         }
-        if (sub_end) {                                           // step 8: accept / reject
-          bool ok = ran && (e <= 1.0);
-          if (ok) {
-            double miny = u[0];
-            KR_FOR(s, 1, S) miny = fmin(miny, u[s]); KR_END
-            if (!(miny >= -o.neg_tol)) ok = false;
-          }
-          if constexpr (KrNet::energy) {
-            constexpr double T_lo = KrNet::T_lo, T_hi = KrNet::T_hi;
-            if (ok && !(u[N - 1] >= T_lo && u[N - 1] <= T_hi)) ok = false;
-          }
-          if (ok && krs_finite(o.chg_max)) {
-            double chg = 0.0;
-            KR_FOR(i, 0, N)
-              const double un = sh.UN(i);
-              chg = fmax(chg, fabs(u[i] - un) / ((i < S) ? (fabs(un) + o.chg_floor) : un));
-            KR_END
-            if (!(chg <= o.chg_max)) ok = false;
-          }
-          if (ok) {
-            n_acc++;
-            KR_FOR(i, 0, N) sh.UN(i) = u[i]; KR_END
-            if (last) cell_done = true;
-            else {
-              t = t + h;
-              if (it <= o.it_fast) h = h * o.grow_fast;
-              else if (it <= o.it_mid) h = h * o.grow_mid;
-            }
-          } else {
-            n_rej++;
-            st |= KR_DST_REJECTED;
-            h = h * o.shrink;
-          }
-          k = 0;
-        }
+        k = 0;
       }
-      if (fail_cell) {                                           // R13: revert
-        c_failed++;
-        c_acc += n_acc; c_rej += n_rej;
-        if (g.status) g.status[cell] = st | KR_DST_FAILED;
-        phase = KRS_FETCH;
-      } else if (cell_done) {                                    // step 9: finalise + layout-out (u == u_n here)
-        c_acc += n_acc; c_rej += n_rej;
-        if (o.finalize) {
-          double rem[E];
-          bool any = false;
-          KR_FOR(nu, 0, E)
-            rem[nu] = 0.0;
-            KR_FOR(s, 0, S)
-              if constexpr (KrNet::comp[nu][s] != 0) { constexpr double cn = (double)KrNet::comp[nu][s]; if (u[s] < 0.0) rem[nu] += cn * u[s]; }
-            KR_END
+    }
+    if (fail_cell) {                                             // R13: revert (the caller's buffers were never written)
+      c_failed++;
+      c_acc += n_acc; c_rej += n_rej;
+      if (g.status) g.status[cell] = st | KR_DST_FAILED;
+      KR_FOR(i, 0, N) u[i] = 1.0; sh.UN(i) = 1.0; KR_END
+      phase = KRS_FETCH;
+    } else if (cell_done) {                                      // step 9: finalise + layout-out (u == u_n here)
+      c_acc += n_acc; c_rej += n_rej;
+      if (o.finalize) {
+        double rem[E];
+        bool any = false;
+        KR_FOR(nu, 0, E)
+          rem[nu] = 0.0;
+          KR_FOR(s, 0, S)
+            if constexpr (KrNet::comp[nu][s] != 0) { constexpr double cn = (double)KrNet::comp[nu][s]; if (u[s] < 0.0) rem[nu] += cn * u[s]; }
           KR_END
-          KR_FOR(s, 0, S) if (u[s] < 0.0) { u[s] = 0.0; st |= KR_DST_CLAMPED_NEG; any = true; } KR_END
-          if (any) {
-            KR_FOR(nu, 0, E)
-              if (rem[nu] != 0.0) {
-                int res = -1;
-                double best = 0.0, cres = 1.0;
-                KR_FOR(s, 0, S)
-                  if constexpr (KrNet::resv[nu][s] != 0) {
-                    constexpr double cn = (double)KrNet::comp[nu][s];
-                    if (res < 0 || u[s] > best) { res = s; best = u[s]; cres = cn; }
-                  }
-                KR_END
-                if (res < 0) st |= KR_DST_NO_RESERVOIR;
-                else {
-                  const double x = best + rem[nu] / cres;
-                  KR_FOR(s, 0, S) if constexpr (KrNet::resv[nu][s] != 0) { if (res == s) u[s] = x; } KR_END
-                  if (x < 0.0) st |= KR_DST_NEEDS_STAGE3;
+        KR_END
+        KR_FOR(s, 0, S) if (u[s] < 0.0) { u[s] = 0.0; st |= KR_DST_CLAMPED_NEG; any = true; } KR_END
+        if (any) {
+          KR_FOR(nu, 0, E)
+            if (rem[nu] != 0.0) {
+              int res = -1;
+              double best = 0.0, cres = 1.0;
+              KR_FOR(s, 0, S)
+                if constexpr (KrNet::resv[nu][s] != 0) {
+                  constexpr double cn = (double)KrNet::comp[nu][s];
+                  if (res < 0 || u[s] > best) { res = s; best = u[s]; cres = cn; }
                 }
+              KR_END
+              if (res < 0) st |= KR_DST_NO_RESERVOIR;
+              else {
+                const double x = best + rem[nu] / cres;
+                KR_FOR(s, 0, S) if constexpr (KrNet::resv[nu][s] != 0) { if (res == s) u[s] = x; } KR_END
+                if (x < 0.0) st |= KR_DST_NEEDS_STAGE3;
               }
-            KR_END
-          }
+            }
+          KR_END
         }
-        KR_FOR(s, 0, S) g.y[cell * S + s] = u[s]; KR_END
-        if constexpr (KrNet::energy) g.T[cell] = u[N - 1];
-        if (g.status) g.status[cell] = st;
-        phase = KRS_FETCH;
       }
+      KR_FOR(s, 0, S) g.y[cell * S + s] = u[s]; KR_END
+      if constexpr (KrNet::energy) g.T[cell] = u[N - 1];
+      if (g.status) g.status[cell] = st;
+      phase = KRS_FETCH;
     }
   }
   unsigned long long c[5] = {c_acc, c_rej, c_newton, c_rate, c_failed};
