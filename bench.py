@@ -36,6 +36,11 @@ from paper_2504_04941_b200 import workloads as w      # noqa: E402
 METRIC = "cell-updates/s for one implicit chem step"
 UNIT = "cell-updates/s"
 
+# DRAM traffic of the step kernel per cell-update, from the ncu --set full captures summarised under profiles/
+# (dram__bytes_read.sum + dram__bytes_write.sum of one launch / cells of that launch).  It is BELOW the algorithmic
+# bytes because the results of the last cells are still in the 126 MB L2 when the kernel ends.
+NCU_DRAM_BYTES_PER_CELL = {("c1", "fp64"): 92.3, ("c3", "fp64"): 300.4}
+
 
 class ClockSampler(threading.Thread):
     """Samples SM clock and throttle reasons through NVML while the timed region runs."""
@@ -232,6 +237,12 @@ def main() -> None:
     restore()
     stats = step(want_stats=True)
     n_failed = stats["n_failed"]
+    mixed_stats = None
+    if mode == B.KR_MIXED:
+        ms = gn.last_mixed_stats()
+        mixed_stats = {"refinements_per_newton": ms["n_refine"] / max(stats["n_newton"], 1),
+                       "fp64_fallback_cell_fraction": ms["n_fp64_cells"] / n_cells,
+                       "fp64_kernel": "register-tile fp64 kernel on the listed cells (second launch)"}
     flops_step = F.step_flops(net, stats)
     kern_ms = float(np.mean(ms_each))                     # this rank's kernel: one launch per step
     achieved_tf = flops_step / (kern_ms * 1e-3) / 1e12
@@ -277,18 +288,23 @@ def main() -> None:
             "dtype": "f64" if mode == B.KR_FP64 else "f32+f64", "data": "synthetic",
             "config": {"workload": w.CONFIG_NAMES[idx], "cells_per_gpu": n_cells, "S": net.n_species, "R": net.n_reac,
                        "N": net.n_unknowns, "dt": cells.dt, "newton": "early-exit, K<=8", "precision_mode": args.mode,
-                       "mapping": {1: "thread-per-cell", 2: "warp-per-cell", 3: "cta-per-cell"}[info["mapping"]],
+                       "mapping": {1: "thread-per-cell", 2: "warp-per-cell", 3: "cta-per-cell", 4: "thread-per-cell (table)",
+                                   5: "group-per-cell (table)"}[info["mapping"]],
+                       "kernel": gn.kernel_desc(),
                        "threads_per_cell": info["threads_per_cell"], "smem_bytes_per_block": info["smem_bytes"],
                        "l2": "state restored from a pristine copy and a 256 MiB buffer written before every timed call",
                        "parallelism": f"cells sharded, {world} rank(s), no data-path collective"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
             "roofline": {"bound": "alu", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
-                         "frac": achieved_tf / peak_tf, "traffic": None,
+                         "frac": achieved_tf / peak_tf,
+                         "traffic": (NCU_DRAM_BYTES_PER_CELL[(f"c{idx}", args.mode)] * n_cells
+                                     if (f"c{idx}", args.mode) in NCU_DRAM_BYTES_PER_CELL else None),
                          "peak_source": "FP64 FMA peak measured in this run (kr_measure_fp64_peak); nominal 148 SM x 64 FMA/clk x 2 x 1.965 GHz = 37.2",
                          "flops_per_launch": flops_step, "kernel_ms": kern_ms,
                          "hbm_bytes_per_launch": bytes_step, "hbm_gbs": bytes_step / (kern_ms * 1e-3) / 1e9},
             "cpu_baseline": cpu,
             "solver": {k: v / n_cells for k, v in stats.items()}, "n_failed": n_failed, "wall_s_timed_region": wall,
+            "mixed": mixed_stats,
         }
         print(json.dumps(line), flush=True)
     if world > 1:

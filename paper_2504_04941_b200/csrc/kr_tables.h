@@ -19,6 +19,12 @@ struct KrDEnt {
   int r, m;
 };
 
+// One term of one Jacobian ENTRY (kr_wpc.cuh assembles J entry by entry): J[dst] = sum_terms coef * D[g0] D[g1] D[g2] D[g3].
+struct KrETerm {
+  double coef;                     // dnu_rs * (+-exponent | third-body efficiency) [* q_ext/k_B on the heat row]
+  unsigned short g0, g1, g2, g3;   // as in KrDEnt
+};
+
 struct KrNetDev {
   int E, S, R, N;        // conservation rows, species, reactions, unknowns (S or S+1)
   int energy;            // 1: T is the last unknown
@@ -58,6 +64,10 @@ struct KrNetDev {
   const int* rprog_ptr;  // [R+1]
   const int* fac;        // [R*6] mass-action factors with powers expanded: 3 forward, 3 reverse species, S = the constant 1
   const int* tgt;        // [R*8] [0] = number of rows the reaction feeds, then (row | (dnu + 128) << 8) with the net dnu
+  int n_entries;         // structurally non-zero entries of J[0..S-1][0..S-1] plus the raw heat row (row S)
+  const int* eprog_ptr;  // [n_entries+1] terms of entry e: eterm[eprog_ptr[e]] .. ; entries sorted by descending term count
+  const int* eprog_dst;  // [n_entries] row * LD + column, LD = (N + 1) | 1
+  const KrETerm* eterm;
 };
 
 struct KrOptsDev {

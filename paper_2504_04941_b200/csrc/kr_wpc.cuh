@@ -256,32 +256,33 @@ __device__ __forceinline__ void rows(const KrNetDev& n, const Cell& c, const Grp
   }
 }
 
-// ---- Jacobian columns (eq. 19): thread <-> column m, one host-built term d = dq_r/dn_m after the other, each scattered
-// to the rows its reaction feeds.  invC = 1 / sum_s y_s chat_s (energy equation only).
-__device__ __forceinline__ void columns(const KrNetDev& n, const Cell& c, const Grp& G, double T, double invC) {
+// ---- Jacobian (eq. 19), thread <-> ENTRY: J[s][m] = sum of its host-built terms dnu_rs dq_r/dn_m, each one multiply
+// chain over the cell's shared-memory block; entries are dealt to the threads longest first, so the threads of a
+// group finish together (column lists are very uneven: an abundant reactant sits in a third of the reactions).
+// No read-modify-write of shared memory, no atomics, fixed order (replaces PAPER.md:232).  J was zeroed by eval().
+__device__ __forceinline__ void entries(const KrNetDev& n, const Cell& c, const Grp& G) {
   const double* D = c.d(0);
+  MT* J = c.m(oMAT);
+  const int nE = n.n_entries;
+  for (int e = G.gl; e < nE; e += GT) {
+    const int p0 = n.eprog_ptr[e], p1 = n.eprog_ptr[e + 1];
+    double acc = 0.0;
+    for (int p = p0; p < p1; ++p) {
+      const KrETerm t = n.eterm[p];
+      acc += t.coef * D[t.g0] * D[t.g1] * D[t.g2] * D[t.g3];
+    }
+    J[n.eprog_dst[e]] = (MT)acc;
+  }
+}
+
+// ---- T row of J (eq. 20 with the dropped dC/dy term, DESIGN.md step 5): thread <-> column m; row S holds the raw heat sum
+__device__ __forceinline__ void trow(const Cell& c, const Grp& G, double T, double invC) {
   double* TH = c.d(oTH);
   MT* J = c.m(oMAT);
   for (int m = G.gl; m < S; m += GT) {
-    for (int i = 0; i < N; ++i) J[i * LD + m] = (MT)0;
-    double heat_dn = 0.0;
-    const int p1 = n.cprog_ptr[m + 1];
-    for (int p = n.cprog_ptr[m]; p < p1; ++p) {
-      const KrDEnt t = n.cprog[p];
-      const double d = t.coef * D[t.g0] * D[t.g1] * D[t.g2] * D[t.g3];
-      const int* tg = n.tgt + 8 * t.r;
-      const int nt = tg[0];
-      for (int q = 0; q < nt; ++q) {
-        const int e = tg[1 + q];
-        J[(e & 255) * LD + m] += (MT)((double)((e >> 8) - 128) * d);
-      }
-      if (ENERGY && KRW_ANY_QEXT) heat_dn += n.qk[t.r] * d;
-    }
-    if (ENERGY) {
-      double acc = 0.0;
-      for (int s = 0; s < S; ++s) acc += TH[S + s] * (double)J[s * LD + m];
-      J[S * LD + m] = (MT)((heat_dn - T * acc) * invC);
-    }
+    double acc = 0.0;
+    for (int s = 0; s < S; ++s) acc += TH[S + s] * (double)J[s * LD + m];
+    J[S * LD + m] = (MT)(((double)J[S * LD + m] - T * acc) * invC);
   }
 }
 
@@ -294,6 +295,10 @@ __device__ __forceinline__ void eval(const KrNetDev& n, const Cell& c, const Grp
   const double invN = krs_rcp(Ncal);
   double *U = c.d(oU), *TH = c.d(oTH), *F = c.d(oF), *NN = c.d(oNN);
   for (int s = G.gl; s <= S; s += GT) NN[s] = (s < S) ? Ncal * U[s] : 1.0;
+  if (wantJ) {
+    MT* Jz = c.m(oMAT);
+    for (int i = G.gl; i < N * LD; i += GT) Jz[i] = (MT)0;
+  }
   G.sync();
   double red[3];
   reactions(n, c, G, invT, lnT, aux0, aux, cell, n_cells, computeK, red[0], red[1]);
@@ -306,8 +311,9 @@ __device__ __forceinline__ void eval(const KrNetDev& n, const Cell& c, const Grp
   const double heat_sum = red[0], heat_dT = red[1];
   const double invC = ENERGY ? krs_rcp(red[2]) : 1.0;
   rows(n, c, G, invN, wantJ);
-  if (wantJ) columns(n, c, G, T, invC);
+  if (wantJ) entries(n, c, G);
   G.sync();
+  if (ENERGY && wantJ) { trow(c, G, T, invC); G.sync(); }
   if (ENERGY) {
     MT* J = c.m(oMAT);
     double r2[3] = {0.0, 0.0, 0.0};
@@ -382,16 +388,18 @@ struct Lane {
 };
 __device__ __forceinline__ int lidx(int row) { return row + row / RB; }     // padded index into a column vector
 
+// executed by EVERY lane of the warp (the row index I is warp-uniform); only the stores are predicated on holding
+// the row, so the warp never splits here
 template <int I>
-__device__ __forceinline__ void publish_row(const MT (&a)[RB][CB], MT (&sc)[RB], int kb, MT* UR, int cg) {
+__device__ __forceinline__ void publish_row(const MT (&a)[RB][CB], MT (&sc)[RB], int kb, MT* UR, int cg, bool holds) {
 #pragma unroll
   for (int j = 0; j < CB; ++j)
-    if (j >= kb) UR[j * NCG + cg] = a[I][j];
-  sc[I] = (MT)-1;                            // the row is used: never a pivot candidate again
+    if (j >= kb) { if (holds) UR[j * NCG + cg] = a[I][j]; }
+  sc[I] = holds ? (MT)-1 : sc[I];            // the row is used: never a pivot candidate again
 }
 
 #define KRW_PUB_CASE(I) \
-  case I: if constexpr (I < RB) publish_row<(I < RB ? I : 0)>(a, sc, kb, UR, L.cg); break;
+  case I: if constexpr (I < RB) publish_row<(I < RB ? I : 0)>(a, sc, kb, UR, L.cg, holds); break;
 
 // pivot key of a candidate: the leading bits of |a| / scale with the row index in the 6 low bits, so that ONE integer
 // maximum gives the scaled pivot of Algorithm 1 and the tie rule (smallest row).  Candidates closer than 2^-46
@@ -460,6 +468,7 @@ __device__ __forceinline__ bool eliminate(const Cell& c, const Grp& G, double h)
   int* PIV = c.i(oPIV);
   int* KOF = c.i(oKOF);
   int* POF = c.i(oPOF);
+  bool fail = false;                          // uniform; no early exit from the column loop (keeps the warp converged)
 #pragma unroll
   for (int kb = 0; kb < CB; ++kb) {
     for (int kc = 0; kc < NCG; ++kc) {
@@ -493,9 +502,10 @@ __device__ __forceinline__ bool eliminate(const Cell& c, const Grp& G, double h)
         if (W > 1 && p < 0 && L.lane == 0) PIV[k & 1] = -1;
       }
       if (W > 1) { G.sync(); p = PIV[k & 1]; }
-      if (p < 0) return false;
-      const int trp = p / RB, ip = p - trp * RB;
-      if (L.tr == trp) {                      // the lanes that hold row p publish it and retire it
+      fail = fail || (p < 0);
+      const int trp = (p >= 0) ? p / RB : 0, ip = (p >= 0) ? p - trp * RB : -1;
+      {                                       // the lanes that hold row p publish it and retire it
+        const bool holds = (L.tr == trp);
         switch (ip) {
           KRW_PUB_CASE(0) KRW_PUB_CASE(1) KRW_PUB_CASE(2) KRW_PUB_CASE(3) KRW_PUB_CASE(4) KRW_PUB_CASE(5) KRW_PUB_CASE(6)
           KRW_PUB_CASE(7) KRW_PUB_CASE(8) KRW_PUB_CASE(9) KRW_PUB_CASE(10) KRW_PUB_CASE(11) KRW_PUB_CASE(12)
@@ -503,12 +513,13 @@ __device__ __forceinline__ bool eliminate(const Cell& c, const Grp& G, double h)
           KRW_PUB_CASE(19) KRW_PUB_CASE(20) KRW_PUB_CASE(21)
           default: break;
         }
-        if (L.cg == 0) { KOF[p] = k; POF[k] = p; }
+        if (holds && L.cg == 0 && ip >= 0) { KOF[p] = k; POF[k] = p; }
       }
       __syncwarp();
       const MT pv = PVS[k & 1];
-      if (!(fabs(pv) >= (MT)(MIXED ? 1e-30 : 1e-300)) || !(fabs(pv) <= (MT)(MIXED ? 3.0e38 : 1.7e308))) return false;
-      const MT rp = mt_rcp(pv);
+      const bool pok = (fabs(pv) >= (MT)(MIXED ? 1e-30 : 1e-300)) && (fabs(pv) <= (MT)(MIXED ? 3.0e38 : 1.7e308));
+      fail = fail || !pok;
+      const MT rp = mt_rcp(pok ? pv : (MT)1);
       if (L.cg == 0 && L.tr == 0) RP[k] = rp;
       MT l[RB], u[CB];
 #pragma unroll
@@ -526,6 +537,7 @@ __device__ __forceinline__ bool eliminate(const Cell& c, const Grp& G, double h)
     }
   }
   G.sync();
+  if (fail) return false;
   constexpr int jN = N / NCG, cgN = N % NCG;  // the right-hand-side column
   if (L.cg == cgN) {
 #pragma unroll
@@ -640,46 +652,45 @@ kr_wpc_kernel(const KrNetDev n, const KrOptsDev o, const KrStepArgs a) {
     for (int s = G.gl; s < S; s += GT) { const double x = a.y[cell * S + s]; UN[s] = x; U[s] = x; }
     if (ENERGY && G.gl == 0) { UN[S] = Tc; U[S] = Tc; }
     G.sync();
-    double t = 0.0, h = a.dt;
+    double t = 0.0, h = a.dt, h_floor = o.h_min_rel * a.dt;
     int n_acc = 0, n_rej = 0;
-    {
-      const double invT = krs_rcp(Tc), lnT = log(Tc);
-      if (!ENERGY) {
-        if (KRW_ANY_REV) { thermo(n, c, G, Tc, invT, lnT); G.sync(); }
-        if (o.h0_mode != 1)            // rate constants (the h0 evaluation below computes them as well)
-          eval(n, c, G, Ncal, Tc, aux0, a.aux, cell, a.n_cells, true, false);
-        c_rate++;
-      }
-      if (o.h0_mode == 1) {
-        if (ENERGY) { thermo(n, c, G, Tc, invT, lnT); G.sync(); c_rate++; }
-        eval(n, c, G, Ncal, Tc, aux0, a.aux, cell, a.n_cells, true, false);
-        double big = 0.0;
-        for (int s = G.gl; s < S; s += GT) {
-          const double x = fabs(F[s]) / (fabs(UN[s]) + o.y_floor);
-          big = (x > big) ? x : big;
-        }
-        big = G.max(big);
-        if (big > 0.0 && finite(big)) h = fmin(a.dt, o.eta / big);
-      }
-    }
-    const double h_floor = o.h_min_rel * fmin(h, a.dt);
+    // The first pass of a cell through the evaluation below is its preliminary evaluation: rate constants of an
+    // isothermal cell, f(u_in) for the first sub-step (step 1, h0_mode 1).  One call site keeps the kernel small.
+    bool prelim = (o.h0_mode == 1) || !ENERGY;
 
     // ---- sub-step loop (steps 6-8) -------------------------------------------------------------------------------
     bool failed = false, handoff = false;
     for (;;) {
-      const double rem = a.dt - t;
       bool last = false;
-      if (h >= rem) { h = rem; last = true; }
-      if (h < h_floor || n_acc + n_rej > o.max_substeps) { failed = true; break; }
-      for (int i = G.gl; i < N; i += GT) U[i] = UN[i];
-      G.sync();
+      if (!prelim) {
+        const double rem = a.dt - t;
+        if (h >= rem) { h = rem; last = true; }
+        if (h < h_floor || n_acc + n_rej > o.max_substeps) { failed = true; break; }
+        for (int i = G.gl; i < N; i += GT) U[i] = UN[i];
+        G.sync();
+      }
       double e = __longlong_as_double(0x7ff0000000000000LL), e_prev = 0.0;
       int it = K + 1;
-      bool ran = true;
+      bool ran = true, was_prelim = false;
       for (int k = 1; k <= K; ++k) {
         const double T = ENERGY ? U[S] : T_iso;
-        if (ENERGY) { thermo(n, c, G, T, krs_rcp(T), log(T)); G.sync(); c_rate++; }
-        eval(n, c, G, Ncal, T, aux0, a.aux, cell, a.n_cells, ENERGY, true);
+        if (ENERGY || (prelim && KRW_ANY_REV)) { thermo(n, c, G, T, krs_rcp(T), log(T)); G.sync(); }
+        if (ENERGY || prelim) c_rate++;
+        eval(n, c, G, Ncal, T, aux0, a.aux, cell, a.n_cells, ENERGY || prelim, !prelim);
+        if (prelim) {
+          if (o.h0_mode == 1) {
+            double big = 0.0;
+            for (int s = G.gl; s < S; s += GT) {
+              const double x = fabs(F[s]) / (fabs(UN[s]) + o.y_floor);
+              big = (x > big) ? x : big;
+            }
+            big = G.max(big);
+            if (big > 0.0 && finite(big)) h = fmin(a.dt, o.eta / big);
+          }
+          h_floor = o.h_min_rel * fmin(h, a.dt);
+          prelim = false; was_prelim = true;
+          break;
+        }
         c_newton++;
         if (!eliminate(c, G, h)) { ran = false; if (MIXED) handoff = a.retry_list != nullptr; break; }
 #if KRW_MIXED
@@ -721,6 +732,7 @@ kr_wpc_kernel(const KrNetDev n, const KrOptsDev o, const KrStepArgs a) {
         e_prev = e;
       }
       if (handoff) break;
+      if (was_prelim) continue;
       // step 8: accept / reject
       bool ok = ran && (e <= 1.0);
       if (ok) {
