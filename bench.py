@@ -39,7 +39,7 @@ UNIT = "cell-updates/s"
 # DRAM traffic of the step kernel per cell-update, from the ncu --set full captures summarised under profiles/
 # (dram__bytes_read.sum + dram__bytes_write.sum of one launch / cells of that launch).  It is BELOW the algorithmic
 # bytes because the results of the last cells are still in the 126 MB L2 when the kernel ends.
-NCU_DRAM_BYTES_PER_CELL = {("c1", "fp64"): 92.3, ("c3", "fp64"): 300.4}
+NCU_DRAM_BYTES_PER_CELL = {("c1", "fp64"): 130.2, ("c3", "fp64"): 285.8}
 
 
 class ClockSampler(threading.Thread):

@@ -274,8 +274,8 @@ class Network:
         return {"n_unknowns": a.value, "mapping": b.value, "threads_per_cell": c.value, "smem_bytes": d.value}
 
     def kernel_desc(self) -> str:
-        buf = C.create_string_buffer(512)
-        _check(load().kr_network_kernel_desc(self._h, buf, 512))
+        buf = C.create_string_buffer(1024)
+        _check(load().kr_network_kernel_desc(self._h, buf, 1024))
         return buf.value.decode()
 
     def last_launch_count(self) -> int:

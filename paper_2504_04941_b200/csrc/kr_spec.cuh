@@ -293,7 +293,7 @@ __device__ __forceinline__ bool krs_lu_solve(const KrsShared& sh, const int (&vh
 
 enum { KRS_FETCH = 0, KRS_RUN = 1, KRS_DONE = 2 };
 
-#ifdef KRS_SYNC
+#if defined(KRS_SYNC) && KRS_SYNC >= 2
 #define KRS_ALIGN() __syncthreads()      // keeps the 8 warps of the block on one instruction stream inside the body too
 #else
 #define KRS_ALIGN() ((void)0)
