@@ -15,7 +15,7 @@ struct KrHostNet {
   std::vector<double> c0, A, beta, Ea, qk, tb, nasa, T_mid;
   // programs of the register-tile kernel (empty when N > 64)
   std::vector<KrDEnt> cprog, rprog;
-  std::vector<int> cprog_ptr, rprog_ptr, fac, tgt, eprog_ptr, eprog_dst;
+  std::vector<int> cprog_ptr, rprog_ptr, fac, tgt, eprog;   // eprog: 4 ints per entry
   std::vector<KrETerm> eterm;
 };
 

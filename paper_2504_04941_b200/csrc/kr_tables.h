@@ -25,6 +25,8 @@ struct KrETerm {
   unsigned short g0, g1, g2, g3;   // as in KrDEnt
 };
 
+static_assert(sizeof(KrETerm) == 16, "KrETerm is read as one 16-byte word");
+
 struct KrNetDev {
   int E, S, R, N;        // conservation rows, species, reactions, unknowns (S or S+1)
   int energy;            // 1: T is the last unknown
@@ -65,8 +67,7 @@ struct KrNetDev {
   const int* fac;        // [R*6] mass-action factors with powers expanded: 3 forward, 3 reverse species, S = the constant 1
   const int* tgt;        // [R*8] [0] = number of rows the reaction feeds, then (row | (dnu + 128) << 8) with the net dnu
   int n_entries;         // structurally non-zero entries of J[0..S-1][0..S-1] plus the raw heat row (row S)
-  const int* eprog_ptr;  // [n_entries+1] terms of entry e: eterm[eprog_ptr[e]] .. ; entries sorted by descending term count
-  const int* eprog_dst;  // [n_entries] row * LD + column, LD = (N + 1) | 1
+  const int4* eprog;     // [n_entries] {first term, number of terms, row * LD + column (LD = (N + 1) | 1), 0}; sorted by descending term count
   const KrETerm* eterm;
 };
 

@@ -264,14 +264,18 @@ __device__ __forceinline__ void entries(const KrNetDev& n, const Cell& c, const 
   const double* D = c.d(0);
   MT* J = c.m(oMAT);
   const int nE = n.n_entries;
+  const uint4* terms = reinterpret_cast<const uint4*>(n.eterm);      // {coef lo, coef hi, g0 | g1 << 16, g2 | g3 << 16}
   for (int e = G.gl; e < nE; e += GT) {
-    const int p0 = n.eprog_ptr[e], p1 = n.eprog_ptr[e + 1];
+    const int4 hd = __ldg(n.eprog + e);
+    const uint4* tp = terms + hd.x;
     double acc = 0.0;
-    for (int p = p0; p < p1; ++p) {
-      const KrETerm t = n.eterm[p];
-      acc += t.coef * D[t.g0] * D[t.g1] * D[t.g2] * D[t.g3];
+#pragma unroll 4
+    for (int p = 0; p < hd.y; ++p) {
+      const uint4 t = __ldg(tp + p);
+      const double coef = __hiloint2double((int)t.y, (int)t.x);
+      acc += coef * D[t.z & 0xffffu] * D[t.z >> 16] * D[t.w & 0xffffu] * D[t.w >> 16];
     }
-    J[n.eprog_dst[e]] = (MT)acc;
+    J[hd.z] = (MT)acc;
   }
 }
 
