@@ -90,8 +90,12 @@ struct KrStepArgs {
   // mixed precision: cells whose fp32 factorisation cannot be refined are appended to retry_list and redone in fp64
   long long* retry_list;               // [n_cells] or null
   unsigned long long* retry_count;     // number of entries appended
-  const long long* list;               // null: cells 0..n_cells-1; else the cells to process ...
+  const long long* list;               // null: cells 0..n_cells-1; else the cells to process, in this order ...
   const unsigned long long* list_count;  // ... and how many of them (device memory)
+  int list_flag;                       // status bits set on every cell of the list (KR_DST_FP64_FALLBACK for the retry pass)
+  // cost pass (stiffest-first scheduling): when non-null the kernel only evaluates f(u_in) and writes the first sub-step
+  // it would take, min(dt, eta / max_s |ydot_s| / (|y_s| + y_floor)), as the cell's key
+  float* cost_out;                     // [n_cells] or null
 };
 
 // status bits (mirror of include/kratos_chem.h, kept numeric so that device code needs no host header)

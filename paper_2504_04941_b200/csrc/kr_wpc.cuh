@@ -646,7 +646,7 @@ kr_wpc_kernel(const KrNetDev n, const KrOptsDev o, const KrStepArgs a) {
     if (cell >= a.n_cells) break;
 
     // ---- step 1: layout-in, clamp, first sub-step -------------------------------------------------
-    int st = a.list ? KR_DST_FP64_FALLBACK : 0;
+    int st = a.list ? a.list_flag : 0;
     double Tc = a.T[cell];
     if (Tc < n.T_lo) { Tc = n.T_lo; st |= KR_DST_T_CLAMPED; }
     if (Tc > n.T_hi) { Tc = n.T_hi; st |= KR_DST_T_CLAMPED; }
@@ -660,7 +660,7 @@ kr_wpc_kernel(const KrNetDev n, const KrOptsDev o, const KrStepArgs a) {
     int n_acc = 0, n_rej = 0;
     // The first pass of a cell through the evaluation below is its preliminary evaluation: rate constants of an
     // isothermal cell, f(u_in) for the first sub-step (step 1, h0_mode 1).  One call site keeps the kernel small.
-    bool prelim = (o.h0_mode == 1) || !ENERGY;
+    bool prelim = (o.h0_mode == 1) || !ENERGY || (a.cost_out != nullptr);
 
     // ---- sub-step loop (steps 6-8) -------------------------------------------------------------------------------
     bool failed = false, handoff = false;
@@ -679,10 +679,10 @@ kr_wpc_kernel(const KrNetDev n, const KrOptsDev o, const KrStepArgs a) {
       for (int k = 1; k <= K; ++k) {
         const double T = ENERGY ? U[S] : T_iso;
         if (ENERGY || (prelim && KRW_ANY_REV)) { thermo(n, c, G, T, krs_rcp(T), log(T)); G.sync(); }
-        if (ENERGY || prelim) c_rate++;
+        if ((ENERGY || prelim) && !a.cost_out) c_rate++;
         eval(n, c, G, Ncal, T, aux0, a.aux, cell, a.n_cells, ENERGY || prelim, !prelim);
         if (prelim) {
-          if (o.h0_mode == 1) {
+          if (o.h0_mode == 1 || a.cost_out) {
             double big = 0.0;
             for (int s = G.gl; s < S; s += GT) {
               const double x = fabs(F[s]) / (fabs(UN[s]) + o.y_floor);
@@ -736,7 +736,10 @@ kr_wpc_kernel(const KrNetDev n, const KrOptsDev o, const KrStepArgs a) {
         e_prev = e;
       }
       if (handoff) break;
-      if (was_prelim) continue;
+      if (was_prelim) {
+        if (a.cost_out) { handoff = true; break; }   // cost pass: the key is the first sub-step
+        continue;
+      }
       // step 8: accept / reject
       bool ok = ran && (e <= 1.0);
       if (ok) {
@@ -772,6 +775,11 @@ kr_wpc_kernel(const KrNetDev n, const KrOptsDev o, const KrStepArgs a) {
         h = h * o.shrink;
         G.sync();
       }
+    }
+    if (handoff && a.cost_out) {
+      if (G.gl == 0) a.cost_out[cell] = (float)h;
+      G.sync();
+      continue;
     }
     if (handoff) {            // the caller's buffers were never written: the fp64 kernel redoes this cell from its input
       if (G.gl == 0) a.retry_list[atomicAdd(a.retry_count, 1ull)] = cell;
