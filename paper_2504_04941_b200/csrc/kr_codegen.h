@@ -15,8 +15,9 @@ struct KrHostNet {
   std::vector<double> c0, A, beta, Ea, qk, tb, nasa, T_mid;
   // programs of the register-tile kernel (empty when N > 64)
   std::vector<KrDEnt> cprog, rprog;
-  std::vector<int> cprog_ptr, rprog_ptr, fac, tgt, eprog;   // eprog: 4 ints per entry
-  std::vector<KrETerm> eterm;
+  std::vector<int> cprog_ptr, rprog_ptr, fac, tgt, emeta[2];
+  int n_entries = 0, elen[2] = {0, 0};
+  std::vector<KrETerm> estream[2];
 };
 
 namespace kr_codegen {

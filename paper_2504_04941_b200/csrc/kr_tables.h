@@ -67,8 +67,12 @@ struct KrNetDev {
   const int* fac;        // [R*6] mass-action factors with powers expanded: 3 forward, 3 reverse species, S = the constant 1
   const int* tgt;        // [R*8] [0] = number of rows the reaction feeds, then (row | (dnu + 128) << 8) with the net dnu
   int n_entries;         // structurally non-zero entries of J[0..S-1][0..S-1] plus the raw heat row (row S)
-  const int4* eprog;     // [n_entries] {first term, number of terms, row * LD + column (LD = (N + 1) | 1), 0}; sorted by descending term count
-  const KrETerm* eterm;
+  // the entry terms as one coalesced stream per thread of a group of 32 (index 0) or 64 (index 1) threads: step i of thread
+  // t reads estream[i * GT + t]; emeta holds row * LD + column (LD = (N + 1) | 1) at the last term of an entry, else -1;
+  // entries are dealt to the threads longest first, padded with zero terms to elen steps
+  const KrETerm* estream[2];
+  const int* emeta[2];
+  int elen[2];
 };
 
 struct KrOptsDev {

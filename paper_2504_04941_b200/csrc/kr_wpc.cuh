@@ -263,19 +263,18 @@ __device__ __forceinline__ void rows(const KrNetDev& n, const Cell& c, const Grp
 __device__ __forceinline__ void entries(const KrNetDev& n, const Cell& c, const Grp& G) {
   const double* D = c.d(0);
   MT* J = c.m(oMAT);
-  const int nE = n.n_entries;
-  const uint4* terms = reinterpret_cast<const uint4*>(n.eterm);      // {coef lo, coef hi, g0 | g1 << 16, g2 | g3 << 16}
-  for (int e = G.gl; e < nE; e += GT) {
-    const int4 hd = __ldg(n.eprog + e);
-    const uint4* tp = terms + hd.x;
-    double acc = 0.0;
+  // {coef lo, coef hi, g0 | g1 << 16, g2 | g3 << 16}: one coalesced 16-byte load per thread and step, no dependent loads
+  const uint4* terms = reinterpret_cast<const uint4*>(n.estream[W - 1]) + G.gl;
+  const int* meta = n.emeta[W - 1] + G.gl;
+  const int len = n.elen[W - 1];
+  double acc = 0.0;
 #pragma unroll 4
-    for (int p = 0; p < hd.y; ++p) {
-      const uint4 t = __ldg(tp + p);
-      const double coef = __hiloint2double((int)t.y, (int)t.x);
-      acc += coef * D[t.z & 0xffffu] * D[t.z >> 16] * D[t.w & 0xffffu] * D[t.w >> 16];
-    }
-    J[hd.z] = (MT)acc;
+  for (int i = 0; i < len; ++i) {
+    const uint4 t = __ldg(terms + i * GT);
+    const int dst = __ldg(meta + i * GT);
+    const double coef = __hiloint2double((int)t.y, (int)t.x);
+    acc += coef * D[t.z & 0xffffu] * D[t.z >> 16] * D[t.w & 0xffffu] * D[t.w >> 16];
+    if (dst >= 0) { J[dst] = (MT)acc; acc = 0.0; }
   }
 }
 
