@@ -404,16 +404,9 @@ __device__ __forceinline__ void publish_row(const MT (&a)[RB][CB], MT (&sc)[RB],
 #define KRW_PUB_CASE(I) \
   case I: if constexpr (I < RB) publish_row<(I < RB ? I : 0)>(a, sc, kb, UR, L.cg, holds); break;
 
-// pivot key of a candidate: the leading bits of |a| / scale with the row index in the 6 low bits, so that ONE integer
-// maximum gives the scaled pivot of Algorithm 1 and the tie rule (smallest row).  Candidates closer than 2^-46
-// (fp64, 64-bit key) / 2^-17 (fp32, 32-bit key) relative count as tied; used rows carry a negative scale and lose.
-#if KRW_MIXED
-typedef int KeyT;
-__device__ __forceinline__ KeyT pivot_key(MT t, int row) { return (__float_as_int(t) | 63) - row; }
-#else
-typedef long long KeyT;
-__device__ __forceinline__ KeyT pivot_key(MT t, int row) { return (__double_as_longlong(t) | 63LL) - (long long)row; }
-#endif
+// Pivot keys: the bits of |a| / scale with the row index in the 6 low bits, so that an integer maximum gives the scaled
+// pivot of Algorithm 1 and its tie rule (smallest row).  Candidates closer than 2^-46 (fp64) / 2^-17 (fp32) relative
+// count as tied; used rows carry a negative scale and lose against every candidate.
 
 // Pass A (thread <-> row): B = -(U - UN - h F), row scales of I - hJ.  Pass B: tiles.  Then N elimination columns.
 // On success X holds the solution of (I - hJ) X = B; in mixed mode the column vectors, reciprocal pivots and the row
@@ -481,21 +474,42 @@ __device__ __forceinline__ bool eliminate(const Cell& c, const Grp& G, double h)
       int p;
       if (W == 1 || L.wq == kc / TC) {        // the warp that holds column k
         const bool mine = (L.tc == kc % TC);
-        KeyT key = (KeyT)-1 << (8 * sizeof(KeyT) - 2);
+        // scaled pivot search (Algorithm 1): the warp-wide integer maximum (REDUX) of the candidates' keys.  fp64: the
+        // high words first, then among the rows that share the largest high word the low words with the row index in
+        // the 6 low bits -- together the 64-bit lexicographic maximum, exact to 2^-46, ties -> smallest row.
+        const int rowbase = L.tr * RB;
+#if KRW_MIXED
+        int key = -2147483647 - 1;
 #pragma unroll
         for (int i = 0; i < RB; ++i) {
           const MT v = a[i][kb];
-          if (mine) Lk[L.tr * RB + i + L.tr] = v;                  // column k as it stands (the multipliers x pivot)
-          const KeyT ki = pivot_key(fabs(v) * sc[i], L.tr * RB + i);
+          if (mine) Lk[rowbase + i + L.tr] = v;                      // column k as it stands (the multipliers x pivot)
+          const int ki = (__float_as_int(fabsf(v) * sc[i]) | 63) - (rowbase + i);
           key = (ki > key) ? ki : key;
         }
+        key = __reduce_max_sync(0xffffffffu, mine ? key : (-2147483647 - 1));
+        p = (key >= 0) ? (63 - (key & 63)) : -1;
+#else
+        int hi[RB], hmax = -2147483647 - 1;
+        unsigned lo[RB];
 #pragma unroll
-        for (int off = TC; off < 32; off <<= 1) {
-          const KeyT k2 = __shfl_xor_sync(0xffffffffu, key, off);
-          key = (k2 > key) ? k2 : key;
+        for (int i = 0; i < RB; ++i) {
+          const MT v = a[i][kb];
+          if (mine) Lk[rowbase + i + L.tr] = v;                      // column k as it stands (the multipliers x pivot)
+          const double t = fabs(v) * sc[i];
+          hi[i] = __double2hiint(t); lo[i] = (unsigned)__double2loint(t);
+          hmax = (hi[i] > hmax) ? hi[i] : hmax;
         }
-        key = __shfl_sync(0xffffffffu, key, kc % TC);              // lane (tr 0, tc of column k) holds the column's maximum
-        p = (key >= 0) ? (63 - (int)(key & 63)) : -1;
+        const int H = __reduce_max_sync(0xffffffffu, mine ? hmax : (-2147483647 - 1));
+        unsigned lk = 0u;
+#pragma unroll
+        for (int i = 0; i < RB; ++i) {
+          const unsigned ki = (lo[i] | 63u) - (unsigned)(rowbase + i);
+          lk = (mine && hi[i] == H && ki > lk) ? ki : lk;
+        }
+        const unsigned Lw = __reduce_max_sync(0xffffffffu, lk);
+        p = (H >= 0) ? (63 - (int)(Lw & 63u)) : -1;
+#endif
         if (mine && p >= 0 && p / RB == L.tr) {                     // the lane that holds a[p][k]
           const int ix = p + L.tr;
           PVS[k & 1] = Lk[ix];
