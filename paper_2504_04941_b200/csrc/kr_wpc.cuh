@@ -10,12 +10,14 @@
 // Work split of one Newton iteration (DESIGN.md steps 2-7) inside the group of 32 W threads that owns a cell:
 //   thermo            : thread <-> species
 //   rate constants, q : thread <-> reaction
-//   Jacobian          : thread <-> COLUMN m, each dq_r/dn_m formed once by the column's owner and scattered down
-//                       the column in shared memory: no atomics (replaces PAPER.md:232), eq. 19 / eq. 20
+//   Jacobian          : thread <-> ENTRY J[s][m]: every entry is the sum of host-built terms dnu_rs dq_r/dn_m, each a
+//                       multiply chain over the cell's shared-memory block; the terms reach each thread as one
+//                       coalesced stream (entries dealt longest first): no atomics, no read-modify-write of shared
+//                       memory, fixed order (replaces PAPER.md:232), eq. 19 / eq. 20
 //   elimination       : the matrix [I - hJ | -G] is spread over the threads as a TR x (TC W) grid of RB x CB
 //                       REGISTER tiles (rows blocked, columns cyclic).  Column k: scaled-pivot search among the
-//                       not yet used rows by the TR lanes that hold the column (shuffles), multipliers and the
-//                       pivot row published through shared memory, rank-1 update of every tile -- RB x CB
+//                       not yet used rows as a warp-wide integer maximum of pivot keys (REDUX), raw column, pivot
+//                       value and pivot row published through shared memory, rank-1 update of every tile -- RB x CB
 //                       independent FMAs per thread and step against RB + CB shared-memory loads.  Rows are never
 //                       exchanged (implicit pivoting: a used row is marked); the update is applied to the used
 //                       rows as well (Gauss-Jordan form of Algorithm 1's elimination), which
@@ -244,8 +246,9 @@ __device__ __forceinline__ void rows(const KrNetDev& n, const Cell& c, const Grp
   for (int s = G.gl; s < S; s += GT) {
     double ys = 0.0, jt = 0.0;
     const int p1 = n.row_ptr[s + 1];
+#pragma unroll 4
     for (int p = n.row_ptr[s]; p < p1; ++p) {
-      const int ent = n.row_ent[p];
+      const int ent = __ldg(n.row_ent + p);
       const int r = ent >> 8;
       const double dnu = (double)((ent & 255) - 128);
       ys += dnu * Q[r];
