@@ -419,47 +419,76 @@ __device__ __forceinline__ bool eliminate(const Cell& c, const Grp& G, double h)
   double *U = c.d(oU), *UN = c.d(oUN), *F = c.d(oF), *B = c.d(oB), *VI = c.d(oVI), *X = c.d(oX);
   MT* J = c.m(oMAT);
   const MT hm = (MT)h;
-  bool rows_ok = true;
-  for (int i = G.gl; i < N; i += GT) {
-    B[i] = -(U[i] - UN[i] - h * F[i]);
-    MT big = (MT)0;
-    bool fin = true;
-    for (int j = 0; j < N; ++j) {
-      const MT x = ((i == j) ? (MT)1 : (MT)0) - hm * J[i * LD + j];
-      const MT ax = fabs(x);
-      big = (ax > big) ? ax : big;
-      fin = fin && (ax <= (MT)(MIXED ? 3.0e38 : 1.7e308));        // false for inf and NaN
-    }
-    const bool ok = fin && (big > (MT)(MIXED ? 1e-30 : 1e-300));
-    rows_ok = rows_ok && ok;
-    VI[i] = ok ? 1.0 / (double)big : 0.0;
-  }
-  rows_ok = G.all(rows_ok);
-  G.sync();
-  if (!rows_ok) return false;
-
+  // Tiles of [I - hJ | -G] straight from J; the row scales (max-norm of each row, Algorithm 1's implicit scaling) are
+  // reduced from the tiles themselves: shuffles across the column groups of a warp, shared memory between two warps.
   MT a[RB][CB];
   MT sc[RB];                                  // > 0: 1 / row scale of a candidate row;  < 0: used or padding row
+  MT big[RB];
+  bool fin = true;
+  constexpr int cgN = N % NCG;                // the column group that holds the right-hand side
 #pragma unroll
   for (int i = 0; i < RB; ++i) {
     const int row = L.tr * RB + i;
     const bool rin = row < N;
-    const double vi = rin ? VI[row] : 0.0;
-    sc[i] = rin ? (MIXED ? (MT)1 : (MT)vi) : (MT)-1;
+    big[i] = (MT)0;
 #pragma unroll
     for (int j = 0; j < CB; ++j) {
       const int col = j * NCG + L.cg;
       MT x = (MT)0;
       if (rin && col < N) {
         x = ((row == col) ? (MT)1 : (MT)0) - hm * J[row * LD + col];
-        if (MIXED) x *= (MT)vi;
+        const MT ax = fabs(x);
+        big[i] = (ax > big[i]) ? ax : big[i];
+        fin = fin && (ax <= (MT)(MIXED ? 3.0e38 : 1.7e308));      // false for inf and NaN
       } else if (rin && col == N) {
-        x = MIXED ? (MT)(B[row] * vi) : (MT)B[row];
+        const double bb = -(U[row] - UN[row] - h * F[row]);
+        B[row] = bb;
+        x = (MT)bb;
       }
       a[i][j] = x;
     }
   }
+#pragma unroll
+  for (int off = 1; off < TC; off <<= 1) {
+#pragma unroll
+    for (int i = 0; i < RB; ++i) {
+      const MT y = __shfl_xor_sync(0xffffffffu, big[i], off);
+      big[i] = (y > big[i]) ? y : big[i];
+    }
+  }
+  if (W > 1) {                                // warp 0 leaves its partial maxima in RS, warp 1 in X (both free here)
+    double* part = (L.wq == 0) ? c.d(oRS) : X;
+    if (L.tc == 0) {
+#pragma unroll
+      for (int i = 0; i < RB; ++i)
+        if (L.tr * RB + i < N) part[L.tr * RB + i] = (double)big[i];
+    }
+    G.sync();
+#pragma unroll
+    for (int i = 0; i < RB; ++i)
+      if (L.tr * RB + i < N) {
+        const MT y0 = (MT)c.d(oRS)[L.tr * RB + i], y1 = (MT)X[L.tr * RB + i];
+        big[i] = (y0 > y1) ? y0 : y1;
+      }
+  }
+  bool rows_ok = fin;
+#pragma unroll
+  for (int i = 0; i < RB; ++i) {
+    const int row = L.tr * RB + i;
+    const bool rin = row < N;
+    const bool ok = big[i] > (MT)(MIXED ? 1e-30 : 1e-300);
+    rows_ok = rows_ok && (ok || !rin);
+    const double vi = (rin && ok) ? krs_rcp((double)big[i]) : 0.0;
+    sc[i] = rin ? (MIXED ? (MT)1 : (MT)vi) : (MT)-1;
+    if (rin && L.cg == 0) VI[row] = vi;
+    if (MIXED) {
+#pragma unroll
+      for (int j = 0; j < CB; ++j) a[i][j] *= (MT)vi;
+    }
+  }
+  rows_ok = G.all(rows_ok);
   G.sync();                                   // J is dead from here on: the mixed mode reuses its space
+  if (!rows_ok) return false;
 
   MT* UR = c.m(oUR);
   MT* RP = c.m(oRP);
@@ -523,6 +552,7 @@ __device__ __forceinline__ bool eliminate(const Cell& c, const Grp& G, double h)
       }
       if (W > 1) { G.sync(); p = PIV[k & 1]; }
       fail = fail || (p < 0);
+      if (G.gl == 0) POF[k] = p;
       const int trp = (p >= 0) ? p / RB : 0, ip = (p >= 0) ? p - trp * RB : -1;
       {                                       // the lanes that hold row p publish it and retire it
         const bool holds = (L.tr == trp);
@@ -533,7 +563,6 @@ __device__ __forceinline__ bool eliminate(const Cell& c, const Grp& G, double h)
           KRW_PUB_CASE(19) KRW_PUB_CASE(20) KRW_PUB_CASE(21)
           default: break;
         }
-        if (holds && L.cg == 0 && ip >= 0) { KOF[p] = k; POF[k] = p; }
       }
       __syncwarp();
       const MT pv = PVS[k & 1];
@@ -558,7 +587,9 @@ __device__ __forceinline__ bool eliminate(const Cell& c, const Grp& G, double h)
   }
   G.sync();
   if (fail) return false;
-  constexpr int jN = N / NCG, cgN = N % NCG;  // the right-hand-side column
+  for (int k = G.gl; k < N; k += GT) KOF[POF[k]] = k;      // the column in which each row was the pivot row
+  G.sync();
+  constexpr int jN = N / NCG;                 // the right-hand-side column
   if (L.cg == cgN) {
 #pragma unroll
     for (int i = 0; i < RB; ++i) {
