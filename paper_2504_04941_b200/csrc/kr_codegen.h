@@ -14,8 +14,8 @@ struct KrHostNet {
   std::vector<int> sp, nu, flags, auxi, dnu_tot, comp, resv, row_ptr, col_ptr, row_ent, col_ent;
   std::vector<double> c0, A, beta, Ea, qk, tb, nasa, T_mid;
   // programs of the register-tile kernel (empty when N > 64)
-  std::vector<KrDEnt> cprog, rprog;
-  std::vector<int> cprog_ptr, rprog_ptr, fac, tgt, emeta[2];
+  std::vector<KrDEnt> rprog;
+  std::vector<int> rprog_ptr, fac, tgt, emeta[2];
   int n_entries = 0, elen[2] = {0, 0};
   std::vector<KrETerm> estream[2];
 };

@@ -60,9 +60,7 @@ struct KrNetDev {
   const int* col_ptr;    // [S+1]  column list of species m
   const int* col_ent;    // packed (reaction << 4) | slot, slot 0..5 = participant slot, 15 = third-body only
   // programs of the register-tile kernel (kr_wpc.cuh); null when N > 64
-  const KrDEnt* cprog;   // derivative terms grouped by column m: cprog_ptr[m] .. cprog_ptr[m+1]
-  const int* cprog_ptr;  // [S+1]
-  const KrDEnt* rprog;   // the same terms grouped by reaction r: rprog_ptr[r] .. rprog_ptr[r+1]
+  const KrDEnt* rprog;   // the derivative terms grouped by reaction r: rprog_ptr[r] .. rprog_ptr[r+1] (mixed-mode residual)
   const int* rprog_ptr;  // [R+1]
   const int* fac;        // [R*6] mass-action factors with powers expanded: 3 forward, 3 reverse species, S = the constant 1
   const int* tgt;        // [R*8] [0] = number of rows the reaction feeds, then (row | (dnu + 128) << 8) with the net dnu

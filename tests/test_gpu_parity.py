@@ -93,6 +93,35 @@ def test_parity_mixed_precision(B, oracle_mod, idx, fixed):
     assert stats["n_newton"] <= 1.6 * ref["stats"]["n_newton"] + 50
 
 
+def test_stiffest_first_scheduling_changes_nothing(B, monkeypatch):
+    """The register-tile launches of several waves run a cost pass, sort the cells by their first sub-step and walk the
+    sorted list; cells are independent, so results, status and counters must be
+    bit-identical to the index-order run, and the extra launches must be counted."""
+    net, cells, opts = w.make_config(3, 9000)                  # > 4 waves of 11 cells x 148 SMs
+    T1, y1, s1, st1, g1 = run_gpu(B, net, cells, opts)
+    assert g1.last_launch_count() == 9                         # cost pass, iota, 6 radix-sort kernels, solve
+    monkeypatch.setenv("KR_NO_LPT", "1")
+    T0, y0, s0, st0, g0 = run_gpu(B, net, cells, opts)
+    assert g0.last_launch_count() == 1
+    np.testing.assert_array_equal(y1, y0)
+    np.testing.assert_array_equal(T1, T0)
+    np.testing.assert_array_equal(s1, s0)
+    assert st1 == st0
+
+
+def test_mixed_fallback_cells_equal_the_fp64_run(B):
+    """A cell the fp32 factorisation cannot resolve is redone from its input by the fp64 kernel: its result must be the
+    fp64 mode's result bit for bit, with KR_ST_FP64_FALLBACK set and nothing else changed."""
+    net, cells, opts = w.make_config(4, 160, fixed_newton=1)
+    T0, y0, s0, st0, _ = run_gpu(B, net, cells, opts)
+    T1, y1, s1, st1, gn = run_gpu(B, net, cells, opts, mode=B.KR_MIXED)
+    fb = (s1 & B.ST_FP64_FALLBACK) != 0
+    assert fb.sum() == gn.last_mixed_stats()["n_fp64_cells"] > 0
+    np.testing.assert_array_equal(y1[fb], y0[fb])
+    np.testing.assert_array_equal(s1[fb] & ~B.ST_FP64_FALLBACK, s0[fb])
+    assert ((s0 & B.ST_FP64_FALLBACK) == 0).all()
+
+
 def test_mixed_precision_needs_a_supported_size(B):
     import torch
     net = w.make_network(4)
