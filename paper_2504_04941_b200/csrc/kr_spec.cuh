@@ -298,6 +298,11 @@ enum { KRS_FETCH = 0, KRS_RUN = 1, KRS_DONE = 2 };
 #else
 #define KRS_ALIGN() ((void)0)
 #endif
+#if defined(KRS_SYNC) && KRS_SYNC >= 3   // a barrier between rate constants and reactions keeps all 4 R rate values live
+#define KRS_ALIGN_RC() __syncthreads()
+#else
+#define KRS_ALIGN_RC() ((void)0)
+#endif
 
 // One trip of the main loop = one pass of EVERY lane through the same straight-line body: rate constants, reactions,
 // Jacobian columns, LU, update, controller.  A lane that has just loaded a cell uses its first pass as the
@@ -384,7 +389,7 @@ kr_spec_kernel(const KrOptsDev o, const KrStepArgs g) {
         double kf[R], kr[R], dlf[R], dlr[R];
         krs_rate_constants<true>(T, aux0, g.aux, active ? cell : 0, g.n_cells, kf, kr, dlf, dlr, uh, ch);
         if (active && !fail_cell) c_rate++;
-        KRS_ALIGN();
+        KRS_ALIGN_RC();
         krs_reactions<true>(Ncal, T, u, kf, kr, dlf, dlr, uh, ch, n, f, a, b, qh, jt, Cv, sc);
       } else {
         double dlf[R], dlr[R];
@@ -396,7 +401,7 @@ kr_spec_kernel(const KrOptsDev o, const KrStepArgs g) {
             c_rate++;
           }
         }
-        KRS_ALIGN();
+        KRS_ALIGN_RC();
         krs_reactions<true>(Ncal, T, u, kfi, kri, dlf, dlr, uh, ch, n, f, a, b, qh, jt, Cv, sc);
       }
       if (active && prelim) {                                    // first sub-step from f(u_in) (step 1, h0_mode 1)
