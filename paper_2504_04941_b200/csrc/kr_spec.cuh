@@ -355,6 +355,20 @@ kr_spec_kernel(const KrOptsDev o, const KrStepArgs g) {
           t = 0.0; h = g.dt; n_acc = 0; n_rej = 0; k = 0;
           h_floor = o.h_min_rel * g.dt;
           pend = (o.h0_mode == 1) || !KrNet::energy;
+#ifdef KRS_PRELIM_WS
+          // isothermal: the preliminary evaluation was done for every cell by kr_spec_prelim_kernel (full warps, no
+          // exponentials in this kernel's body, no discarded pass)
+          KR_FOR(r, 0, R)
+            constexpr int fl = KrNet::flags[r];
+            constexpr double A_r = KrNet::A[r];
+            if constexpr (fl & KR_DF_CONST) kfi[r] = A_r; else kfi[r] = g.prelim[(long long)r * g.n_cells + cell];
+            if constexpr (fl & KR_DF_REV) kri[r] = g.prelim[(long long)(R + r) * g.n_cells + cell]; else kri[r] = 0.0;
+          KR_END
+          h = g.prelim[(long long)(2 * R) * g.n_cells + cell];
+          h_floor = o.h_min_rel * fmin(h, g.dt);
+          pend = false;
+          c_rate++;
+#endif
         }
       }
     }
@@ -393,6 +407,7 @@ kr_spec_kernel(const KrOptsDev o, const KrStepArgs g) {
         krs_reactions<true>(Ncal, T, u, kf, kr, dlf, dlr, uh, ch, n, f, a, b, qh, jt, Cv, sc);
       } else {
         double dlf[R], dlr[R];
+#ifndef KRS_PRELIM_WS
         if (__any_sync(0xffffffffu, active && prelim)) {         // rate constants of freshly loaded isothermal cells
           double kf[R], kr[R];
           krs_rate_constants<false>(T, aux0, g.aux, active ? cell : 0, g.n_cells, kf, kr, dlf, dlr, uh, ch);
@@ -401,6 +416,7 @@ kr_spec_kernel(const KrOptsDev o, const KrStepArgs g) {
             c_rate++;
           }
         }
+#endif
         KRS_ALIGN_RC();
         krs_reactions<true>(Ncal, T, u, kfi, kri, dlf, dlr, uh, ch, n, f, a, b, qh, jt, Cv, sc);
       }
@@ -549,3 +565,37 @@ kr_spec_kernel(const KrOptsDev o, const KrStepArgs g) {
     atomicAdd(g.stats + 3, c[2]); atomicAdd(g.stats + 4, c[3]); atomicAdd(g.stats + 5, c[4]);
   }
 }
+
+#ifdef KRS_PRELIM_WS
+// Preliminary evaluation of an isothermal network for every cell (DESIGN.md step 1): rate constants at the clamped T and
+// the first sub-step from f(u_in).  One thread per cell, grid-stride, full warps; output as [2R + 1][n_cells].
+extern "C" __global__ void __launch_bounds__(256) kr_spec_prelim_kernel(const KrOptsDev o, const KrStepArgs g) {
+  constexpr int S = KrNet::S, R = KrNet::R, N = KrNet::N;
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x; cell < g.n_cells; cell += stride) {
+    double Tc = g.T[cell];
+    constexpr double T_lo = KrNet::T_lo, T_hi = KrNet::T_hi;
+    Tc = (Tc < T_lo) ? T_lo : ((Tc > T_hi) ? T_hi : Tc);
+    const double Ncal = g.rho[cell] * (1.0 / KR_M_U);
+    const double aux0 = (KrNet::n_aux > 0) ? g.aux[cell] : 0.0;
+    double u[N];
+    KR_FOR(s, 0, S) u[s] = g.y[cell * S + s]; KR_END
+    double kf[R], kr[R], dlf[R], dlr[R], uh[S], ch[S];
+    krs_rate_constants<false>(Tc, aux0, g.aux, cell, g.n_cells, kf, kr, dlf, dlr, uh, ch);
+    double h = g.dt;
+    if (o.h0_mode == 1) {
+      double n[S], f[N], a[R], b[R], qh[R], jt[N], Cv = 1.0, sc = 0.0;
+      krs_reactions<false>(Ncal, Tc, u, kf, kr, dlf, dlr, uh, ch, n, f, a, b, qh, jt, Cv, sc);
+      double big = 0.0;
+      KR_FOR(s, 0, S) big = fmax(big, fabs(f[s]) / (fabs(u[s]) + o.y_floor)); KR_END
+      if (big > 0.0 && krs_finite(big)) h = fmin(g.dt, o.eta / big);
+    }
+    KR_FOR(r, 0, R)
+      constexpr int fl = KrNet::flags[r];
+      if constexpr (!(fl & KR_DF_CONST)) g.prelim[(long long)r * g.n_cells + cell] = kf[r];
+      if constexpr (fl & KR_DF_REV) g.prelim[(long long)(R + r) * g.n_cells + cell] = kr[r];
+    KR_END
+    g.prelim[(long long)(2 * R) * g.n_cells + cell] = h;
+  }
+}
+#endif

@@ -98,6 +98,9 @@ struct KrStepArgs {
   // cost pass (stiffest-first scheduling): when non-null the kernel only evaluates f(u_in) and writes the first sub-step
   // it would take, min(dt, eta / max_s |ydot_s| / (|y_s| + y_floor)), as the cell's key
   float* cost_out;                     // [n_cells] or null
+  // isothermal networks, specialised thread-per-cell kernel: rate constants and first sub-step of every cell, written by
+  // kr_spec_prelim_kernel as [2R + 1][n_cells] (k_f rows, k_r rows, h0), read by the solve kernel when it loads a cell
+  double* prelim;
 };
 
 // status bits (mirror of include/kratos_chem.h, kept numeric so that device code needs no host header)
