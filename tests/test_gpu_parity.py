@@ -122,6 +122,26 @@ def test_mixed_fallback_cells_equal_the_fp64_run(B):
     assert ((s0 & B.ST_FP64_FALLBACK) == 0).all()
 
 
+@pytest.mark.parametrize("idx", [3, 4])
+def test_full_size_sampled_mixed(B, oracle_mod, idx):
+    """Mixed precision at BASELINE size in the launch configuration bench.py times (stiffest-first order, fp32 kernel,
+    fp64 kernel on the retry list): sampled cells against the fp64 oracle at 1e-5, every cell finite, non-negative and
+    conserving."""
+    net, cells, opts = w.make_config(idx)
+    n = cells.n_cells
+    T, y, st, stats, gn = run_gpu(B, net, cells, opts, mode=B.KR_MIXED)
+    ms = gn.last_mixed_stats()
+    ok = (st & 8) == 0
+    assert ok.mean() > 0.999 and np.isfinite(y).all() and (y >= 0).all()
+    assert ms["n_fp64_cells"] == int(((st & B.ST_FP64_FALLBACK) != 0).sum())
+    drift = P.element_drift(net, cells.y[ok], y[ok]).max(axis=1)
+    assert (drift > 1e-12).mean() <= 1e-4 and drift.max() <= 1e-9, float(drift.max())
+    pick = np.sort(np.random.default_rng(199 + idx).choice(n, size={3: 160, 4: 48}[idx], replace=False))
+    ref = P.oracle_reference(oracle_mod, net, cells.take(pick), opts)
+    out = P.compare(net, ref, T[pick], y[pick], st[pick] & ~B.ST_FP64_FALLBACK, tol=MIXED_TOL, allow_path_flips=MIXED_FLIPS[idx])
+    print(f"full-size mixed config {idx}: {out} mixed={ms}")
+
+
 def test_mixed_precision_needs_a_supported_size(B):
     import torch
     net = w.make_network(4)
