@@ -672,9 +672,14 @@ kr_wpc_kernel(const KrNetDev n, const KrOptsDev o, const KrStepArgs a) {
   extern __shared__ __align__(16) char kr_sm_raw[];
   const int K = o.max_newton;
   Grp G;
-  G.g = threadIdx.x / GT; G.gl = threadIdx.x % GT;
   Cell c;
+#if KRW_CPB == 1
+  G.g = 0; G.gl = threadIdx.x;                // one cell per block: every shared-memory offset is a compile-time constant
+  c.base = kr_sm_raw;
+#else
+  G.g = threadIdx.x / GT; G.gl = threadIdx.x % GT;
   c.base = kr_sm_raw + (size_t)G.g * CELL_BYTES;
+#endif
   G.red = c.d(oRED);
   volatile long long* cellslot = (volatile long long*)(c.d(oRED) + 8 * W);
   double *U = c.d(oU), *UN = c.d(oUN), *F = c.d(oF), *X = c.d(oX);
