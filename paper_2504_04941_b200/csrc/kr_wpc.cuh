@@ -187,28 +187,45 @@ __device__ __forceinline__ void reactions(const KrNetDev& n, const Cell& c, cons
   double *NN = c.d(oNN), *TH = c.d(oTH), *KF = c.d(oKF), *KR = c.d(oKR), *Q = c.d(oQ);
   heat_sum = 0.0; heat_dT = 0.0;
   for (int r = G.gl; r < R; r += GT) {
-    const int fl = n.flags[r];
+    // every table value of the reaction is requested up front: independent loads, one exposed latency instead of a chain
+    const int fl = __ldg(n.flags + r);
+    const int2* fp = reinterpret_cast<const int2*>(n.fac + 6 * r);
+    const int2 f01 = __ldg(fp), f23 = __ldg(fp + 1), f45 = __ldg(fp + 2);
+    const double A_r = __ldg(n.A + r);
+    const double qk = KRW_ANY_QEXT ? __ldg(n.qk + r) : 0.0;
+    double beta = 0.0, Ea = 0.0, c0 = 0.0;
+    int dn_tot = 0;
+    int4 tg0 = make_int4(0, 0, 0, 0), tg1 = make_int4(0, 0, 0, 0);
+    if (computeK) {
+      beta = __ldg(n.beta + r); Ea = __ldg(n.Ea + r); c0 = __ldg(n.c0 + r);
+      if (KRW_ANY_REV) {
+        dn_tot = __ldg(n.dnu_tot + r);
+        const int4* tp = reinterpret_cast<const int4*>(n.tgt + 8 * r);
+        tg0 = __ldg(tp); tg1 = __ldg(tp + 1);
+      }
+    }
     double kf, kr = 0.0, dlf = 0.0, dlr = 0.0;
     if (computeK) {
-      if (fl & KR_DF_CONST) kf = n.A[r];
+      if (fl & KR_DF_CONST) kf = A_r;
       else if (fl & KR_DF_AUX) {
         const int ai = n.auxi[r];
-        kf = n.A[r] * (ai > 0 ? aux[(long long)ai * n_cells + cell] : aux0);
+        kf = A_r * (ai > 0 ? aux[(long long)ai * n_cells + cell] : aux0);
       } else {
-        const double beta = n.beta[r], Ea = n.Ea[r];
-        const double lnkf = n.c0[r] + beta * lnT - Ea * invT;
+        const double lnkf = c0 + beta * lnT - Ea * invT;
         kf = krs_exp(lnkf);
         dlf = (beta + Ea * invT) * invT;
-        if (fl & KR_DF_REV) {
+        if (KRW_ANY_REV && (fl & KR_DF_REV)) {
           double sg = 0.0, su = 0.0;
-          const int nt = n.tgt[8 * r];
-          for (int t = 0; t < nt; ++t) {
-            const int e = n.tgt[8 * r + 1 + t];
-            const double cf = (double)((e >> 8) - 128);
-            sg += cf * TH[e & 255];
-            su += cf * TH[S + (e & 255)];
-          }
-          const double lnKc = -sg + (double)n.dnu_tot[r] * (n.ln_p0_kB - lnT);
+          const int tg[8] = {tg0.x, tg0.y, tg0.z, tg0.w, tg1.x, tg1.y, tg1.z, tg1.w};
+#pragma unroll
+          for (int t = 0; t < 7; ++t)
+            if (t < tg[0]) {
+              const int e = tg[1 + t];
+              const double cf = (double)((e >> 8) - 128);
+              sg += cf * TH[e & 255];
+              su += cf * TH[S + (e & 255)];
+            }
+          const double lnKc = -sg + (double)dn_tot * (n.ln_p0_kB - lnT);
           kr = krs_exp(lnkf - lnKc);
           dlr = dlf - su * invT;
         }
@@ -217,9 +234,8 @@ __device__ __forceinline__ void reactions(const KrNetDev& n, const Cell& c, cons
     } else {
       kf = KF[r]; kr = KR[r];
     }
-    const int* fc = n.fac + 6 * r;
-    const double Pf = NN[fc[0]] * NN[fc[1]] * NN[fc[2]];
-    const double Pr = NN[fc[3]] * NN[fc[4]] * NN[fc[5]];
+    const double Pf = NN[f01.x] * NN[f01.y] * NN[f23.x];
+    const double Pr = NN[f23.y] * NN[f45.x] * NN[f45.y];
     double Mtb = 1.0;
     const double qhat = kf * Pf - kr * Pr;
     if (KRW_ANY_TB && (fl & KR_DF_TB)) {
@@ -229,7 +245,6 @@ __device__ __forceinline__ void reactions(const KrNetDev& n, const Cell& c, cons
     }
     const double q = Mtb * qhat;
     Q[r] = q;
-    const double qk = KRW_ANY_QEXT ? n.qk[r] : 0.0;
     heat_sum += qk * q;
     if (ENERGY) {
       const double dqdT = Mtb * (kf * dlf * Pf - kr * dlr * Pr);
