@@ -93,6 +93,30 @@ def test_parity_mixed_precision(B, oracle_mod, idx, fixed):
     assert stats["n_newton"] <= 1.6 * ref["stats"]["n_newton"] + 50
 
 
+@pytest.mark.parametrize("S,energy,n_rev,mode", [(13, 1, 10, 0), (24, 0, 90, 0), (24, 0, 90, 1), (40, 1, 150, 0), (47, 1, 200, 0),
+                                                  (63, 1, 260, 0), (63, 1, 260, 1), (64, 1, 260, 0)])
+def test_register_tile_kernel_on_other_sizes(B, oracle_mod, S, energy, n_rev, mode):
+    """Sizes between the BASELINE configs: every tile shape the host can pick (one warp up to 48 doubles per thread, two
+    warps above, the energy equation on a warp pair, N = 64 and N = 65 -> shared-memory kernel) against the oracle, fp64
+    and mixed, on seeded astro-like networks of the config-3 recipe."""
+    rng = np.random.default_rng(4242 + 100 * S + energy)
+    net = w._network_random(rng, 3, 5, S, n_rev, 10, 10, energy, reversible=False)
+    w._check_conservation(net)
+    cells = w.make_cells(3, net, 61, seed=977 + S)
+    opts = w.default_opts(3, fixed_newton=1)
+    ref = P.oracle_reference(oracle_mod, net, cells, opts)
+    T, y, st, stats, gn = run_gpu(B, net, cells, opts, mode=mode)
+    desc = gn.kernel_desc()
+    N = S + energy
+    assert ("register-tile" in desc) == (N <= 64), desc
+    out = P.compare(net, ref, T, y, st & ~B.ST_FP64_FALLBACK, tol=MIXED_TOL if mode else P.TOL,
+                    allow_path_flips=0.03 if mode else 0.0)
+    print(f"S={S} energy={energy} mode={mode}: {desc[:90]} {out}")
+    assert out["n_comparable"] >= 0.6 * out["n"], out      # random thermochemistry: more cells fp64 itself does not resolve
+    ok = (st & 8) == 0
+    assert P.element_drift(net, cells.y[ok], y[ok]).max() <= (1e-9 if mode else 1e-12)
+
+
 def test_stiffest_first_scheduling_changes_nothing(B, monkeypatch):
     """The register-tile launches of several waves run a cost pass, sort the cells by their first sub-step and walk the
     sorted list; cells are independent, so results, status and counters must be
