@@ -153,6 +153,8 @@ def main() -> None:
     ap.add_argument("--mode", default="fp64", choices=["fp64", "mixed"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cells", type=int, default=0, help="override the cell count (testing only)")
+    ap.add_argument("--mapping", type=int, default=0, help="override the per-cell mapping (KR_MAP_*; mapping study only)")
+    ap.add_argument("--threads-per-cell", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -186,6 +188,8 @@ def main() -> None:
     cells = w.make_cells(idx, net, n_cells, seed=w.BASE_SEED + 1000 + idx + 7919 * rank)
     opts = w.default_opts(idx, fixed_newton=0)
     gn = B.Network(net, opts)
+    if args.mapping:
+        gn.set_mapping(args.mapping, args.threads_per_cell)
     stream = torch.cuda.current_stream()
     gn.set_stream(stream.cuda_stream)
 
