@@ -117,6 +117,19 @@ def test_register_tile_kernel_on_other_sizes(B, oracle_mod, S, energy, n_rev, mo
     assert P.element_drift(net, cells.y[ok], y[ok]).max() <= (1e-9 if mode else 1e-12)
 
 
+@pytest.mark.parametrize("idx,n,mode", [(1, 3000, 0), (2, 5000, 0), (3, 2500, 0), (3, 2500, 1), (4, 400, 0), (4, 400, 1)])
+def test_results_are_deterministic(B, idx, n, mode):
+    """Fixed summation orders, no atomics on the data path: repeated calls give identical bits, whatever the order in which
+    the persistent kernels happen to pick up the cells (a shared-memory race would show here)."""
+    net, cells, opts = w.make_config(idx, n)
+    runs = [run_gpu(B, net, cells, opts, mode=mode) for _ in range(3)]
+    for T, y, st, stats, _ in runs[1:]:
+        np.testing.assert_array_equal(y, runs[0][1])
+        np.testing.assert_array_equal(T, runs[0][0])
+        np.testing.assert_array_equal(st, runs[0][2])
+        assert stats == runs[0][3]
+
+
 def test_stiffest_first_scheduling_changes_nothing(B, monkeypatch):
     """The register-tile launches of several waves run a cost pass, sort the cells by their first sub-step and walk the
     sorted list; cells are independent, so results, status and counters must be
