@@ -41,7 +41,7 @@ constexpr double EXP_CLAMP = 690.0;         // R18
 
 enum : int32_t { F_REV = 1, F_TB = 2, F_CONST = 4, F_AUX = 8 };
 enum : int32_t { ST_REJECTED_ONCE = 1, ST_CLAMPED_NEG = 2, ST_FAILED_REVERTED = 8, ST_T_CLAMPED = 16,
-                 ST_NO_RESERVOIR = 32, ST_NEEDS_STAGE3 = 64 };
+                 ST_NO_RESERVOIR = 32, ST_NEEDS_STAGE3 = 64, ST_STAGE3 = 128 };
 
 template <class R> struct real_of { using type = R; };
 template <class R> struct real_of<std::complex<R>> { using type = R; };
@@ -326,6 +326,8 @@ inline bool finite_all(const Real* x, int n) {
 
 struct Counters { int64_t acc = 0, rej = 0, newton = 0, lu = 0, rate = 0, failed = 0; };
 
+template <class Real> int finalize_state(const kr_oracle_network& n, Real* un, double* margin);
+
 inline void margin_update(double* m, double a, double b) {
   if (!m) return;
   const double den = std::max(std::fabs(a), std::fabs(b));
@@ -481,35 +483,108 @@ int32_t step_cell(const kr_oracle_network& n, double rho, double& T_io, double* 
     return st | ST_FAILED_REVERTED;                      // T_io, y_io untouched
   }
 
-  // step 9: finalise (PAPER.md:212-216 stages 1-2).  Stage 1: negatives -> 0.  Stage 2 "corrects the
-  // violation in element abundances brought by step 1": the amount stage 1 added to row nu,
-  // -sum_s N_{nu,s} min(y_s, 0), is taken back from that row's reservoir species (reading R12: equal to the
-  // paper's initial-minus-final element totals up to the solver's own conservation error, which is rounding;
-  // forming it from the clamped amounts keeps a trace reservoir from absorbing eps * total).
-  if (o.finalize) {
-    std::vector<Real> removed(E, Real(0));
-    bool any = false;
-    for (int s = 0; s < S; ++s)
-      if (w.un[s] < Real(0)) {
-        for (int nu = 0; nu < E; ++nu) removed[nu] += Real(n.comp[size_t(nu) * S + s]) * w.un[s];
-        w.un[s] = Real(0); st |= ST_CLAMPED_NEG; any = true;
-      }
-    for (int nu = 0; any && nu < E; ++nu) {
-      if (removed[nu] == Real(0)) continue;
-      int res = -1, second = -1;
-      for (int s = 0; s < S; ++s) {
-        if (!n.reservoir_candidates[size_t(nu) * S + s]) continue;
-        if (res < 0 || w.un[s] > w.un[res]) { second = res; res = s; }
-        else if (second < 0 || w.un[s] > w.un[second]) second = s;
-      }
-      if (res < 0) { st |= ST_NO_RESERVOIR; continue; }
-      if (second >= 0) margin_update(margin, double(w.un[res]), double(w.un[second]));
-      w.un[res] = w.un[res] + removed[nu] / Real(n.comp[size_t(nu) * S + res]);
-      if (w.un[res] < Real(0)) st |= ST_NEEDS_STAGE3;
-    }
-  }
+  if (o.finalize) st |= finalize_state<Real>(n, w.un.data(), margin);
   for (int s = 0; s < S; ++s) y_io[s] = double(w.un[s]);
   if (n.energy) T_io = double(w.un[S]);
+  return st;
+}
+
+// Step 9: post-processing of the final state.
+//   Stage 1: negatives -> 0.
+//   Stage 2 "corrects the violation in element abundances brought by step 1": the amount stage 1 added
+//     to row nu, -sum_s N_{nu,s} min(y_s, 0), is taken back from that row's reservoir species -- the single-row species
+//     with the largest abundance (reading R12: equal to the paper's initial-minus-final element totals up to the
+//     solver's own conservation error, which is rounding; forming it from the clamped amounts keeps a trace reservoir
+//     from absorbing eps * total).
+//   Stage 3 (reading R23): "if step 2 causes negative abundances in some single-element species, the
+//     most abundant compound species is disintegrated into elements just sufficiently to correct this".  For every
+//     element row whose reservoir went negative, in row order: need = -y_res N_{nu,res} atoms; the neutral compound
+//     (>= 2 non-zero rows, no entry on a signed row) with the largest abundance that contains the element gives up
+//     z = min(y_c, need / N_{nu,c}); its atoms of every row go to that row's reservoir; repeated with the next most
+//     abundant compound until the need is met (the reservoir then ends at exactly 0) or no compound is left (the
+//     NEEDS_STAGE3 bit stays).  Every row total is unchanged by construction.
+// Returns the status bits it sets.  un has S entries (abundances only).
+template <class Real>
+int finalize_state(const kr_oracle_network& n, Real* un, double* margin) {
+  const int E = n.E, S = n.S;
+  int st = 0;
+  std::vector<Real> removed(E, Real(0));
+  std::vector<int> res_of(E, -1);
+  bool any = false;
+  for (int s = 0; s < S; ++s)
+    if (un[s] < Real(0)) {
+      for (int nu = 0; nu < E; ++nu) removed[nu] += Real(n.comp[size_t(nu) * S + s]) * un[s];
+      un[s] = Real(0); st |= ST_CLAMPED_NEG; any = true;
+    }
+  if (!any) return st;
+  auto reservoir = [&](int nu, int* second_out) {
+    int res = -1, second = -1;
+    for (int s = 0; s < S; ++s) {
+      if (!n.reservoir_candidates[size_t(nu) * S + s]) continue;
+      if (res < 0 || un[s] > un[res]) { second = res; res = s; }
+      else if (second < 0 || un[s] > un[second]) second = s;
+    }
+    if (second_out) *second_out = second;
+    return res;
+  };
+  bool need3 = false;
+  for (int nu = 0; nu < E; ++nu) {
+    if (removed[nu] == Real(0)) continue;
+    int second = -1;
+    const int res = reservoir(nu, &second);
+    if (res < 0) { st |= ST_NO_RESERVOIR; continue; }
+    if (second >= 0) margin_update(margin, double(un[res]), double(un[second]));
+    res_of[nu] = res;
+    un[res] = un[res] + removed[nu] / Real(n.comp[size_t(nu) * S + res]);
+    if (un[res] < Real(0)) need3 = true;
+  }
+  if (!need3) return st;
+  // stage 3
+  std::vector<char> signed_row(E, 0), compound(S, 0);
+  for (int nu = 0; nu < E; ++nu)
+    for (int s = 0; s < S; ++s)
+      if (n.comp[size_t(nu) * S + s] < 0) signed_row[nu] = 1;
+  for (int s = 0; s < S; ++s) {
+    int rows = 0;
+    bool neutral = true;
+    for (int nu = 0; nu < E; ++nu)
+      if (n.comp[size_t(nu) * S + s] != 0) { rows++; if (signed_row[nu]) neutral = false; }
+    compound[s] = (rows >= 2 && neutral) ? 1 : 0;
+  }
+  for (int nu = 0; nu < E; ++nu) {
+    const int res = res_of[nu];
+    if (res < 0 || !(un[res] < Real(0))) continue;
+    const Real nres = Real(n.comp[size_t(nu) * S + res]);
+    if (signed_row[nu] || !(nres > Real(0))) { st |= ST_NEEDS_STAGE3; continue; }
+    Real need = -un[res] * nres;
+    for (int iter = 0; iter < S && need > Real(0); ++iter) {
+      int c = -1;
+      for (int s = 0; s < S; ++s) {
+        if (!compound[s] || n.comp[size_t(nu) * S + s] <= 0 || !(un[s] > Real(0))) continue;
+        bool placeable = true;                     // every other row of the compound needs a reservoir for its atoms
+        for (int mu = 0; mu < E && placeable; ++mu)
+          if (mu != nu && n.comp[size_t(mu) * S + s] != 0 && res_of[mu] < 0 && reservoir(mu, nullptr) < 0) placeable = false;
+        if (!placeable) continue;
+        if (c < 0 || un[s] > un[c]) c = s;
+      }
+      if (c < 0) break;
+      const Real nc = Real(n.comp[size_t(nu) * S + c]);
+      Real z = need / nc;
+      const bool all = !(z < un[c]);
+      if (all) z = un[c];
+      un[c] = all ? Real(0) : un[c] - z;
+      for (int mu = 0; mu < E; ++mu) {
+        const int nm = n.comp[size_t(mu) * S + c];
+        if (nm == 0 || mu == nu) continue;
+        if (res_of[mu] < 0) res_of[mu] = reservoir(mu, nullptr);
+        un[res_of[mu]] = un[res_of[mu]] + Real(nm) * z / Real(n.comp[size_t(mu) * S + res_of[mu]]);
+      }
+      un[res] = un[res] + nc * z / nres;
+      need = all ? need - nc * z : Real(0);
+    }
+    if (need > Real(0)) st |= ST_NEEDS_STAGE3;
+    else { un[res] = Real(0); st |= ST_STAGE3; }   // "just sufficiently": the reservoir ends at exactly zero
+  }
   return st;
 }
 
@@ -691,6 +766,13 @@ int kr_oracle_lu_solve(int32_t nn, double* M, const double* b, double* x, int32_
   if (!lu_factor<double>(nn, M, v.data(), perm)) return -1;
   for (int i = 0; i < nn; ++i) x[i] = b[i];
   lu_substitute<double>(nn, M, perm, x);
+  return 0;
+}
+
+int kr_oracle_finalize(kr_oracle_network* n, double* y, int32_t* status) {
+  if (!n || !y) return -1;
+  const int st = finalize_state<double>(*n, y, nullptr);
+  if (status) *status = st;
   return 0;
 }
 

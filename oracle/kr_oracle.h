@@ -78,6 +78,9 @@ int kr_oracle_lu_solve(int32_t n, double* M, const double* b, double* x, int32_t
 /* step 6: one backward-Euler sub-step of size h from u_n = (y[, T]); u_out [N];
  * e_out = last e_k, it_out = first k with e_k <= 1 (K+1 if none); returns 0, or 1 when the
  * sub-step aborted (LU failure / non-finite / bail-out). */
+/* Post-processing stages 1-3 applied to one state y[S] in place; *status receives the bits set. */
+int kr_oracle_finalize(kr_oracle_network*, double* y, int32_t* status);
+
 int kr_oracle_be_substep(kr_oracle_network*, double rho, double T, const double* y, const double* aux_cell,
                          double h, double* u_out, double* e_out, int32_t* it_out);
 

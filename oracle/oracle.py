@@ -68,6 +68,7 @@ def load():
     lib.kr_oracle_eval_rhs_complex.argtypes = [vp, C.c_double, C.c_double, C.c_double, _dp, _dp, _dp, _dp, _dp]
     lib.kr_oracle_eval_jacobian.argtypes = [vp, C.c_double, C.c_double, _dp, _dp, _dp]
     lib.kr_oracle_lu_solve.argtypes = [C.c_int32, _dp, _dp, _dp, _ip]
+    lib.kr_oracle_finalize.argtypes = [vp, _dp, C.POINTER(C.c_int32)]
     lib.kr_oracle_be_substep.argtypes = [vp, C.c_double, C.c_double, _dp, _dp, C.c_double, _dp, _dp, _ip]
     _lib = lib
     return lib
@@ -184,6 +185,15 @@ class OracleNetwork:
         ax = _f64(np.zeros(1) if aux_cell is None else aux_cell)
         load().kr_oracle_eval_jacobian(self._h, float(rho), float(T), _d(_f64(y)), _d(ax), _d(J))
         return J
+
+    def finalize(self, y):
+        """Post-processing stages 1-3 on one state; returns (y_out, status bits)."""
+        yy = _f64(np.asarray(y, dtype=np.float64)).copy()
+        st = C.c_int32(0)
+        rc = load().kr_oracle_finalize(self._h, _d(yy), C.byref(st))
+        if rc != 0:
+            raise RuntimeError("oracle finalize failed")
+        return yy, int(st.value)
 
     def be_substep(self, rho: float, T: float, y, h: float, aux_cell=None):
         u = np.zeros(self.N)

@@ -482,3 +482,88 @@ def test_controller_bookkeeping(oracle_mod):
     T, y, st, stats, _ = on2.step(H.cells_of(1e6 * M_U, 300.0, yin, 1.0e9))
     assert st[0] & 8 and stats["n_failed"] == 1
     np.testing.assert_array_equal(y, yin)
+
+
+# ---- P11: post-processing stages 1-3 (readings R12 / R23) -------------------------------------------
+def _post_net():
+    # elements a, b; species: a, b, a2 (single-element, a row), ab, ab2 (compounds); one reaction keeps the network valid
+    return H.tiny_network([[1, 0, 2, 1, 1], [0, 1, 0, 1, 2]], [((0, 1), (3,), 1e-10, 0.0, 0.0, 0, -1)])
+
+
+def test_P11_stages_1_2_restore_what_stage_1_added(oracle_mod):
+    """Stage 1 zeroes negatives, stage 2 takes the amount that added to each element from the largest single-element
+    species of that element; computed here with exact fractions."""
+    on = oracle_mod.OracleNetwork(_post_net(), w.SolverOpts())
+    y = np.array([0.30, 0.20, 0.05, -0.01, 0.40])           # ab negative: stage 1 adds 0.01 a and 0.01 b
+    yo, st = on.finalize(y)
+    exp = [Fraction(30, 100) - Fraction(1, 100), Fraction(20, 100) - Fraction(1, 100), Fraction(5, 100), 0, Fraction(40, 100)]
+    assert st == 2                                           # CLAMPED_NEG only
+    np.testing.assert_allclose(yo, [float(x) for x in exp], rtol=0, atol=6e-17)
+    # the reservoir is the LARGEST single-element species: with a2 > a the a-row correction goes to a2 (2 atoms each)
+    y2 = np.array([0.01, 0.20, 0.30, -0.02, 0.40])
+    yo2, st2 = on.finalize(y2)
+    np.testing.assert_allclose(yo2, [0.01, 0.18, 0.30 - 0.02 / 2, 0.0, 0.40], rtol=0, atol=6e-17)
+    # nothing negative: untouched, no bits
+    y3 = np.array([0.1, 0.2, 0.3, 0.0, 0.4])
+    yo3, st3 = on.finalize(y3)
+    assert st3 == 0 and np.array_equal(yo3, y3)
+
+
+def test_P11_stage_3_disintegrates_the_most_abundant_compound_just_enough(oracle_mod):
+    net = _post_net()
+    on = oracle_mod.OracleNetwork(net, w.SolverOpts())
+    comp = net.composition.astype(np.float64)
+    # stage 1 clamps ab (-0.05): stage 2 wants 0.05 a from `a` (0.01) and 0.05 b from `b` (0.30): `a` goes to -0.04.
+    y = np.array([0.01, 0.30, 0.005, -0.05, 0.40])
+    yo, st = on.finalize(y)
+    assert st == (2 | 128), st                               # CLAMPED_NEG | STAGE3, NEEDS_STAGE3 cleared
+    assert yo.min() >= 0.0
+    np.testing.assert_allclose(comp @ yo, comp @ y, rtol=0, atol=6e-17)     # every element total unchanged
+    # the most abundant compound holding `a` is ab2 (0.40): it gives up exactly 0.04 molecules -> 0.04 a and 0.08 b;
+    # the a reservoir ends at exactly zero, ab stays clamped, a2 is untouched
+    np.testing.assert_allclose(yo, [0.0, 0.30 - 0.05 + 0.08, 0.005, 0.0, 0.40 - 0.04], rtol=0, atol=6e-17)
+    assert yo[0] == 0.0
+    # not enough of ab2: it is used up, then the next compound (none left but ab = 0) -> NEEDS_STAGE3 stays, totals still hold
+    y2 = np.array([0.01, 0.30, 0.005, -0.05, 0.03])
+    yo2, st2 = on.finalize(y2)
+    assert st2 & 64 and not (st2 & 128)
+    np.testing.assert_allclose(comp @ yo2, comp @ y2, rtol=0, atol=6e-17)
+    assert yo2[4] == 0.0 and yo2[0] < 0.0
+    # two compounds needed: ab2 (0.03) is exhausted, ab (0.02) covers the remaining 0.01
+    y3 = np.array([0.01, 0.30, 0.005, 0.02, 0.03])
+    y3n = y3.copy(); y3n[2] = -0.025                          # a2 negative: stage 2 takes 0.05 a from `a`
+    yo3, st3 = on.finalize(y3n)
+    assert st3 == (2 | 128) and yo3.min() >= 0.0
+    np.testing.assert_allclose(comp @ yo3, comp @ y3n, rtol=0, atol=6e-17)
+    np.testing.assert_allclose(yo3, [0.0, 0.30 + 0.06 + 0.01, 0.0, 0.01, 0.0], rtol=0, atol=6e-17)
+
+
+def test_P11_stage_3_leaves_charged_compounds_alone(oracle_mod):
+    """Config 2 has only ions as multi-row species: nothing to disintegrate, the flag stays (R23)."""
+    net = w.make_network(2)
+    on = oracle_mod.OracleNetwork(net, w.default_opts(2))
+    y = np.array([1e-6, 0.5, 0.4, 0.05, -0.2, 0.01])          # H, H+, e-, He, He+ (negative), He++
+    yo, st = on.finalize(y)
+    comp = net.composition.astype(np.float64)
+    np.testing.assert_allclose(comp @ yo, comp @ y, rtol=0, atol=1e-16)
+    assert (st & 64) and not (st & 128) and yo[3] < 0.0
+
+
+def test_P11_random_states_conserve_and_end_non_negative(oracle_mod):
+    net = w.make_network(3)
+    on = oracle_mod.OracleNetwork(net, w.default_opts(3))
+    comp = net.composition.astype(np.float64)
+    rng = np.random.default_rng(11)
+    n3 = 0
+    for _ in range(300):
+        y = 10.0 ** rng.uniform(-8, -3, net.n_species)
+        neg = rng.choice(net.n_species, size=rng.integers(1, 4), replace=False)
+        y[neg] *= -rng.uniform(0.1, 30.0, neg.size)
+        yo, st = on.finalize(y)
+        tot, tot0 = comp @ yo, comp @ y
+        assert np.max(np.abs(tot - tot0) / np.abs(comp @ np.abs(y))) < 1e-14
+        if st & 128:
+            n3 += 1
+        if not (st & (32 | 64)):
+            assert yo.min() >= 0.0
+    assert n3 >= 20                                           # stage 3 was exercised
