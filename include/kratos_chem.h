@@ -7,7 +7,7 @@
  *   abundances plus temperature (eqs. 18-20), integrated by an implicit
  *   ("semi-implicit") scheme with adaptive sub-steps, each
  *   Newton iteration solving one small dense system by LU with implicit-scaled row pivoting
- *   (Algorithm 1), followed by the post-processing repair stages 1-2 and the
+ *   (Algorithm 1), followed by the post-processing repair stages 1-3 and the
  *   retry / revert policy.  Readings of everything the paper leaves open are
  *   listed in DESIGN.md ("Readings R1-R22").
  *
@@ -45,7 +45,8 @@ enum { KR_ST_REJECTED_ONCE = 1,    /* at least one sub-step was rejected and ret
        KR_ST_FAILED_REVERTED = 8,  /* controller gave up; the cell's T and y are left as given (R13) */
        KR_ST_T_CLAMPED = 16,       /* input T was outside [T_lo, T_hi] and was clamped */
        KR_ST_NO_RESERVOIR = 32,    /* stage 2: a conservation row has no single-element species */
-       KR_ST_NEEDS_STAGE3 = 64 };  /* stage 2 drove the reservoir negative (stage 3 is not built) */
+       KR_ST_NEEDS_STAGE3 = 64,    /* stage 2 drove a reservoir negative and stage 3 found no neutral compound to disintegrate */
+       KR_ST_STAGE3 = 128 };       /* stage 3 disintegrated compound species to refill a reservoir */
 
 /* precision_mode */
 enum { KR_FP64 = 0,    /* everything in fp64 */
@@ -92,7 +93,7 @@ typedef struct {
   double grow_fast, grow_mid; /* h <- h * grow_fast if it <= it_fast, * grow_mid if it <= it_mid */
   double chg_floor, chg_max;  /* optional accuracy limiter; off when chg_max = +inf */
   int32_t it_fast, it_mid, max_substeps;
-  int32_t finalize;     /* 1: run post-processing stages 1-2; 0: skip */
+  int32_t finalize;     /* 1: run post-processing stages 1-3; 0: skip */
   double h_min_rel;     /* fail when h < h_min_rel * (first sub-step size) */
   double bail_ratio;    /* early-exit mode: abort the sub-step when e_k > bail_ratio * e_{k-1}, k >= 2 */
 } kr_solver_opts;

@@ -11,7 +11,7 @@
 struct KrHostNet {
   int E = 0, S = 0, R = 0, N = 0, energy = 0, n_aux = 0, any_rev = 0, any_tb = 0, any_qext = 0;
   double T_lo = 0, T_hi = 0, ln_p0_kB = 0;
-  std::vector<int> sp, nu, flags, auxi, dnu_tot, comp, resv, row_ptr, col_ptr, row_ent, col_ent;
+  std::vector<int> sp, nu, flags, auxi, dnu_tot, comp, resv, compound, signed_row, row_ptr, col_ptr, row_ent, col_ent;
   std::vector<double> c0, A, beta, Ea, qk, tb, nasa, T_mid;
   // programs of the register-tile kernel (empty when N > 64)
   std::vector<KrDEnt> rprog;
@@ -79,6 +79,8 @@ inline std::string net_header(const KrHostNet& H, int block, int min_blocks) {
   s += arr1("double", "T_mid", H.T_mid, H.S, fd);
   s += arr2("int", "comp", H.comp, H.E, H.S, fi);
   s += arr2("int", "resv", H.resv, H.E, H.S, fi);
+  s += arr1("int", "compound", H.compound, H.S, fi);
+  s += arr1("int", "signed_row", H.signed_row, H.E, fi);
   s += "};\n";
   return s;
 }

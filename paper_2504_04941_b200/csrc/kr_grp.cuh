@@ -14,6 +14,7 @@
 // The kernel is persistent: a group that finishes a cell pulls the next one from the global counter.
 #pragma once
 #include "kr_device.cuh"
+#include "kr_post.cuh"
 
 struct KrGrpLayout {
   int oM, oU, oUN, oF, oB, oV, oTH, oKF, oKR, oQ, oDQT, oQH, oMT, oRED, total;   // in doubles
@@ -481,34 +482,9 @@ __global__ void __launch_bounds__(256) kr_grp_kernel(const KrNetDev n, const KrO
       G.sync();
       continue;
     }
-    // ---- step 9: finalise (serial in thread 0: O(E S) once per cell) + layout-out ------------------
+    // ---- step 9: finalise (stages 1-3, kr_post.cuh; serial in thread 0: O(E S) once per cell) + layout-out ------------------
     if (o.finalize && G.gl == 0) {
-      bool any = false;
-      for (int nu = 0; nu < E; ++nu) {
-        double rem = 0.0;
-        for (int s = 0; s < S; ++s) {
-          const double x = c[L.oUN + s];
-          if (x < 0.0) rem += (double)n.comp[nu * S + s] * x;
-        }
-        c[L.oB + nu] = rem;
-      }
-      for (int s = 0; s < S; ++s)
-        if (c[L.oUN + s] < 0.0) { c[L.oUN + s] = 0.0; st |= KR_DST_CLAMPED_NEG; any = true; }
-      for (int nu = 0; any && nu < E; ++nu) {
-        const double rem = c[L.oB + nu];
-        if (rem == 0.0) continue;
-        int res = -1;
-        double best = 0.0;
-        for (int s = 0; s < S; ++s) {
-          if (!n.resv[nu * S + s]) continue;
-          const double x = c[L.oUN + s];
-          if (res < 0 || x > best) { res = s; best = x; }
-        }
-        if (res < 0) { st |= KR_DST_NO_RESERVOIR; continue; }
-        const double x = best + rem / (double)n.comp[nu * S + res];
-        c[L.oUN + res] = x;
-        if (x < 0.0) st |= KR_DST_NEEDS_STAGE3;
-      }
+      st |= kr_postprocess(KrPostTab{n}, [&](int s) -> double& { return c[L.oUN + s]; });
       if (a.status) a.status[cell] = st;
     } else if (G.gl == 0 && a.status) {
       a.status[cell] = st;

@@ -19,6 +19,7 @@
 #pragma once
 #include "kr_tables.h"
 #include "kr_math.cuh"
+#include "kr_post.cuh"
 
 template <int I> struct KrIC { static constexpr int value = I; };
 template <int B, int E, class F>
@@ -291,6 +292,20 @@ __device__ __forceinline__ bool krs_lu_solve(const KrsShared& sh, const int (&vh
   return ok;                                               // no early exit: every lane of the block walks the same code
 }
 
+// step 9 on the lane's u_n in shared memory ([entry][lane] layout), out of line: it runs once per cell and only when an
+// abundance ended negative
+struct KrsPostTab {
+  __device__ __forceinline__ int E() const { return KrNet::E; }
+  __device__ __forceinline__ int S() const { return KrNet::S; }
+  __device__ __forceinline__ int comp(int nu, int s) const { return KrNet::comp[nu][s]; }
+  __device__ __forceinline__ int resv(int nu, int s) const { return KrNet::resv[nu][s]; }
+  __device__ __forceinline__ int compound(int s) const { return KrNet::compound[s]; }
+  __device__ __forceinline__ int signed_row(int nu) const { return KrNet::signed_row[nu]; }
+};
+__device__ __noinline__ int krs_post(double* un0) {
+  return kr_postprocess(KrsPostTab{}, [&](int s) -> double& { return un0[s * KRS_BLOCK]; });
+}
+
 enum { KRS_FETCH = 0, KRS_RUN = 1, KRS_DONE = 2 };
 
 #if defined(KRS_SYNC) && KRS_SYNC >= 2
@@ -516,35 +531,12 @@ kr_spec_kernel(const KrOptsDev o, const KrStepArgs g) {
       phase = KRS_FETCH;
     } else if (cell_done) {                                      // step 9: finalise + layout-out (u == u_n here)
       c_acc += n_acc; c_rej += n_rej;
-      if (o.finalize) {
-        double rem[E];
+      if (o.finalize) {                                          // post-processing stages 1-3
         bool any = false;
-        KR_FOR(nu, 0, E)
-          rem[nu] = 0.0;
-          KR_FOR(s, 0, S)
-            if constexpr (KrNet::comp[nu][s] != 0) { constexpr double cn = (double)KrNet::comp[nu][s]; if (u[s] < 0.0) rem[nu] += cn * u[s]; }
-          KR_END
-        KR_END
-        KR_FOR(s, 0, S) if (u[s] < 0.0) { u[s] = 0.0; st |= KR_DST_CLAMPED_NEG; any = true; } KR_END
-        if (any) {
-          KR_FOR(nu, 0, E)
-            if (rem[nu] != 0.0) {
-              int res = -1;
-              double best = 0.0, cres = 1.0;
-              KR_FOR(s, 0, S)
-                if constexpr (KrNet::resv[nu][s] != 0) {
-                  constexpr double cn = (double)KrNet::comp[nu][s];
-                  if (res < 0 || u[s] > best) { res = s; best = u[s]; cres = cn; }
-                }
-              KR_END
-              if (res < 0) st |= KR_DST_NO_RESERVOIR;
-              else {
-                const double x = best + rem[nu] / cres;
-                KR_FOR(s, 0, S) if constexpr (KrNet::resv[nu][s] != 0) { if (res == s) u[s] = x; } KR_END
-                if (x < 0.0) st |= KR_DST_NEEDS_STAGE3;
-              }
-            }
-          KR_END
+        KR_FOR(s, 0, S) any = any || (u[s] < 0.0); KR_END
+        if (any) {                                               // rare: the shared routine works on u_n (== u here)
+          st |= krs_post(&sh.UN(0));
+          KR_FOR(s, 0, S) u[s] = sh.UN(s); KR_END
         }
       }
       KR_FOR(s, 0, S) g.y[cell * S + s] = u[s]; KR_END

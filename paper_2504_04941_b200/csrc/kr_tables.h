@@ -54,6 +54,8 @@ struct KrNetDev {
   // conservation rows
   const int* comp;       // [E*S]
   const int* resv;       // [E*S] 1 where species s is a reservoir candidate of row nu
+  const int* compound;   // [S] 1: neutral compound (>= 2 non-zero rows, none of them signed): stage-3 candidate (R23)
+  const int* signed_row; // [E] 1: the row has negative entries (a charge row)
   // gather lists of the group (warp / CTA per cell) kernels
   const int* row_ptr;    // [S+1]  row list of species s: entries row_ptr[s]..row_ptr[s+1]
   const int* row_ent;    // packed (reaction << 8) | (dnu + 128)
@@ -111,6 +113,7 @@ struct KrStepArgs {
 #define KR_DST_T_CLAMPED 16
 #define KR_DST_NO_RESERVOIR 32
 #define KR_DST_NEEDS_STAGE3 64
+#define KR_DST_STAGE3 128
 
 #define KR_DF_REV 1
 #define KR_DF_TB 2

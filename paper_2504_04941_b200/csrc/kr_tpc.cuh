@@ -8,6 +8,7 @@
 // atomic), so lanes never idle while cells remain (a8, "refill").
 #pragma once
 #include "kr_device.cuh"
+#include "kr_post.cuh"
 
 #define KR_TPC_MAX_N 16
 #define KR_TPC_BD 64
@@ -345,34 +346,7 @@ __global__ void __launch_bounds__(KR_TPC_BD) kr_tpc_kernel(const KrNetDev n, con
         phase = KR_PH_FETCH;
       } else if (cell_done) {                                    // step 9: finalise + layout-out
         c_acc += n_acc; c_rej += n_rej;
-        if (o.finalize) {
-          bool any = false;
-          for (int nu = 0; nu < E; ++nu) {
-            double rem = 0.0;
-            for (int s = 0; s < S; ++s) {
-              const double x = v.at(v.oUN, s);
-              if (x < 0.0) rem += (double)n.comp[nu * S + s] * x;
-            }
-            v.at(v.oB, nu) = rem;
-          }
-          for (int s = 0; s < S; ++s)
-            if (v.at(v.oUN, s) < 0.0) { v.at(v.oUN, s) = 0.0; st |= KR_DST_CLAMPED_NEG; any = true; }
-          for (int nu = 0; any && nu < E; ++nu) {
-            const double rem = v.at(v.oB, nu);
-            if (rem == 0.0) continue;
-            int res = -1;
-            double best = 0.0;
-            for (int s = 0; s < S; ++s) {
-              if (!n.resv[nu * S + s]) continue;
-              const double x = v.at(v.oUN, s);
-              if (res < 0 || x > best) { res = s; best = x; }
-            }
-            if (res < 0) { st |= KR_DST_NO_RESERVOIR; continue; }
-            const double x = best + rem / (double)n.comp[nu * S + res];
-            v.at(v.oUN, res) = x;
-            if (x < 0.0) st |= KR_DST_NEEDS_STAGE3;
-          }
-        }
+        if (o.finalize) st |= kr_postprocess(KrPostTab{n}, [&](int s) -> double& { return v.at(v.oUN, s); });
         for (int s = 0; s < S; ++s) a.y[cell * S + s] = v.at(v.oUN, s);
         if (ENERGY) a.T[cell] = v.at(v.oUN, S);
         if (a.status) a.status[cell] = st;

@@ -33,6 +33,7 @@
 #pragma once
 #include "kr_tables.h"
 #include "kr_math.cuh"
+#include "kr_post.cuh"
 
 #ifndef KRW_REF_MAX
 #define KRW_REF_MAX 5          // most refinement passes per Newton iteration (mixed mode)
@@ -860,35 +861,9 @@ kr_wpc_kernel(const KrNetDev n, const KrOptsDev o, const KrStepArgs a) {
       G.sync();
       continue;
     }
-    // ---- step 9: finalise (PAPER.md:212-216 stages 1-2; serial in thread 0, O(E S) once per cell) + layout-out -------
+    // ---- step 9: finalise (PAPER.md:212-216 stages 1-3, kr_post.cuh; serial in thread 0, once per cell) + layout-out ----
     if (o.finalize && G.gl == 0) {
-      double* RW = c.d(oB);
-      bool any = false;
-      for (int nu = 0; nu < E; ++nu) {
-        double rem = 0.0;
-        for (int s = 0; s < S; ++s) {
-          const double x = UN[s];
-          if (x < 0.0) rem += (double)n.comp[nu * S + s] * x;
-        }
-        RW[nu] = rem;
-      }
-      for (int s = 0; s < S; ++s)
-        if (UN[s] < 0.0) { UN[s] = 0.0; st |= KR_DST_CLAMPED_NEG; any = true; }
-      for (int nu = 0; any && nu < E; ++nu) {
-        const double rem = RW[nu];
-        if (rem == 0.0) continue;
-        int res = -1;
-        double best = 0.0;
-        for (int s = 0; s < S; ++s) {
-          if (!n.resv[nu * S + s]) continue;
-          const double x = UN[s];
-          if (res < 0 || x > best) { res = s; best = x; }
-        }
-        if (res < 0) { st |= KR_DST_NO_RESERVOIR; continue; }
-        const double x = best + rem / (double)n.comp[nu * S + res];
-        UN[res] = x;
-        if (x < 0.0) st |= KR_DST_NEEDS_STAGE3;
-      }
+      st |= kr_postprocess(KrPostTab{n}, [&](int s) -> double& { return UN[s]; });
       if (a.status) a.status[cell] = st;
     } else if (G.gl == 0 && a.status) {
       a.status[cell] = st;

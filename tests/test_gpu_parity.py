@@ -282,6 +282,42 @@ def test_T_clamp_revert_and_repair_paths(B, oracle_mod):
     assert ((st & 2) != 0).sum() >= 3
 
 
+@pytest.mark.parametrize("idx,mapping,tpc", [(0, None, 0), (1, None, 0), (3, None, 0), (4, None, 0), (1, 4, 1), (3, 5, 32), (3, 3, 64)])
+def test_post_processing_stage_3(B, oracle_mod, idx, mapping, tpc):
+    """Stages 1-3 of the post-processing (R23) in every kernel family against the oracle: inputs with a
+    strongly negative compound and an almost empty reservoir, a step too short to change them and a tolerance that accepts
+    them, so that what comes back is the post-processed input -- clamped, refilled from the reservoir, and the reservoir
+    refilled by disintegrating the most abundant compound."""
+    net, cells, opts = w.make_config(idx, 96, fixed_newton=1)
+    comp = net.composition
+    rng = np.random.default_rng(5 + idx)
+    rows = (comp != 0).sum(axis=0)
+    compounds = np.nonzero((rows >= 2) & (comp >= 0).all(axis=0))[0]
+    assert compounds.size >= 1
+    y = np.abs(cells.y).copy() + 1e-12
+    for c in range(cells.n_cells):
+        neg = compounds[rng.integers(compounds.size)]
+        e = np.nonzero(comp[:, neg])[0][0]                       # its first element: empty that element's reservoirs
+        for s in range(net.n_species):
+            if comp[e, s] != 0 and rows[s] == 1:
+                y[c, s] *= 1e-9
+        others = [s for s in compounds if s != neg and comp[e, s] > 0]
+        scale = max([y[c, s] * comp[e, s] for s in others], default=y[c].max()) / comp[e, neg]
+        y[c, neg] = -rng.uniform(0.1, 1.6) * scale               # < 1: one compound suffices, > 1: several are needed
+    cells.y = y
+    cells.dt = cells.dt * 1e-40
+    opts.neg_tol = 1e30
+    To, yo, sto, statso, _ = oracle_mod.OracleNetwork(net, opts).step(cells)
+    assert ((sto & 128) != 0).sum() >= (20 if idx else 0) and ((sto & 8) == 0).all()     # config 0 has a single compound
+    T, yg, st, stats, gn = run_gpu(B, net, cells, opts, mapping=mapping, tpc=tpc)
+    np.testing.assert_array_equal(st, sto)
+    assert P.rel_err(yg, yo).max() <= 1e-12
+    done = ((st & 128) != 0) & ((st & 64) == 0)                 # every negative reservoir could be refilled
+    assert (yg[done] >= 0).all()
+    tot = np.abs(y) @ np.abs(comp.T).astype(np.float64)
+    assert (np.abs((yg - y) @ comp.T.astype(np.float64)) / tot).max() <= 1e-14
+
+
 def test_argument_errors(B):
     import torch
     net, cells, opts = w.make_config(2, 8)
