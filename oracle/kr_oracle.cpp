@@ -2,8 +2,8 @@
 //
 // What it is: a plain, slow, obviously-correct, single-threaded C++17 restatement of
 //   PAPER.md:143-150 (eq. 15, the ODE system), 158-163 (eq. 16, Arrhenius; reading R4),
-//   173-187 (eqs. 18-20, analytic Jacobian), 199 (T limits), 212-218 (post-processing stages 1-2,
-//   retry/revert), 236-276 (Algorithm 1: Crout LU with implicit-scaled row pivoting; reading R14),
+//   173-187 (eqs. 18-20, analytic Jacobian), 199 (T limits), 212-218 (post-processing stages 1-3: readings
+//   R12 / R23; revert on persistent failure: R13), 236-276 (Algorithm 1: Crout LU with implicit-scaled row pivoting; reading R14),
 //   423 (7-coefficient thermo polynomials),
 // in the order and notation of SURVEY.md 8(c) steps 1-9 (= DESIGN.md "Algorithm").  Dense N x N arrays,
 // reaction-index summation order, no blocking, no fusion, no reordering.  `double` throughout; the same
@@ -17,9 +17,11 @@
 // P3 detailed balance against K_c recomputed in numpy, P4 element conservation, P5 LU vs
 // numpy.linalg.solve / Cramer, P6 analytic J vs complex-step, P7 H ionisation-balance quadratic
 // (eq. 35 with eq. 36 coefficients), P8 K=1 equals u_n + h (I-hJ)^-1 f(u_n),
-// P9 adiabatic energy drift O(h^2), P10 long-double witness.
+// P9 adiabatic energy drift O(h^2), P10 long-double witness, P11 post-processing stages 1-3 (exact fractions on a
+// five-species network, row totals, minimal disintegration, charged compounds left alone).
 // Parity unpinned: the controller constants of step 8 and the choice of Jacobian
-// approximations (dropped dC terms) -- the paper does not publish them.
+// approximations (dropped dC terms) -- the paper does not publish them.  The two-level retry of PAPER.md:218 is not
+// restated: a cell whose controller gives up is reverted after its first attempt.
 #include "kr_oracle.h"
 
 #include <algorithm>
