@@ -327,7 +327,7 @@ __device__ __forceinline__ bool kr_grp_lu_solve(const KrGrpLayout& L, double* c,
 template <bool ENERGY, int W>
 __global__ void __launch_bounds__(256) kr_grp_kernel(const KrNetDev n, const KrOptsDev o, const KrStepArgs a) {
   extern __shared__ double kr_sm[];
-  const int S = n.S, N = n.N, E = n.E, K = o.max_newton, ld = n.ld;
+  const int S = n.S, N = n.N, K = o.max_newton, ld = n.ld;
   const int GT = 32 * W;
   const KrGrpLayout L = kr_grp_layout(N, S, n.R, ld, n.energy, n.any_tb, W);
   KrGrp<W> G;

@@ -187,7 +187,7 @@ __device__ __forceinline__ bool kr_tpc_lu_solve(const KrTpcView& v, int N) {
 template <bool ENERGY>
 __global__ void __launch_bounds__(KR_TPC_BD) kr_tpc_kernel(const KrNetDev n, const KrOptsDev o, const KrStepArgs a) {
   extern __shared__ double kr_sm[];
-  const int S = n.S, R = n.R, N = n.N, E = n.E, K = o.max_newton;
+  const int S = n.S, R = n.R, N = n.N, K = o.max_newton;
   const int lane = threadIdx.x & 31;
   KrTpcView v;
   v.sm = kr_sm; v.tid = threadIdx.x; v.BD = blockDim.x;
