@@ -46,7 +46,8 @@ enum { KR_ST_REJECTED_ONCE = 1,    /* at least one sub-step was rejected and ret
        KR_ST_T_CLAMPED = 16,       /* input T was outside [T_lo, T_hi] and was clamped */
        KR_ST_NO_RESERVOIR = 32,    /* stage 2: a conservation row has no single-element species */
        KR_ST_NEEDS_STAGE3 = 64,    /* stage 2 drove a reservoir negative and stage 3 found no neutral compound to disintegrate */
-       KR_ST_STAGE3 = 128 };       /* stage 3 disintegrated compound species to refill a reservoir */
+       KR_ST_STAGE3 = 128,         /* stage 3 disintegrated compound species to refill a reservoir */
+       KR_ST_RETRIED = 256 };      /* the first attempt failed; the result (or the revert) is the second attempt's */
 
 /* precision_mode */
 enum { KR_FP64 = 0,    /* everything in fp64 */
@@ -96,6 +97,9 @@ typedef struct {
   int32_t finalize;     /* 1: run post-processing stages 1-3; 0: skip */
   double h_min_rel;     /* fail when h < h_min_rel * (first sub-step size) */
   double bail_ratio;    /* early-exit mode: abort the sub-step when e_k > bail_ratio * e_{k-1}, k >= 2 */
+  int32_t retry;        /* 1: a cell whose first attempt fails is redone from its input with tightened control before it is
+                         * reverted (R24): one more launch on the listed cells.  Default 0. */
+  double retry_h0;      /* factor on the first sub-step of the second attempt (default 0.01) */
 } kr_solver_opts;
 
 /* Work counters of one call, summed over cells. */

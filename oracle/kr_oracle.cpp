@@ -43,7 +43,7 @@ constexpr double EXP_CLAMP = 690.0;         // R18
 
 enum : int32_t { F_REV = 1, F_TB = 2, F_CONST = 4, F_AUX = 8 };
 enum : int32_t { ST_REJECTED_ONCE = 1, ST_CLAMPED_NEG = 2, ST_FAILED_REVERTED = 8, ST_T_CLAMPED = 16,
-                 ST_NO_RESERVOIR = 32, ST_NEEDS_STAGE3 = 64, ST_STAGE3 = 128 };
+                 ST_NO_RESERVOIR = 32, ST_NEEDS_STAGE3 = 64, ST_STAGE3 = 128, ST_RETRIED = 256 };
 
 template <class R> struct real_of { using type = R; };
 template <class R> struct real_of<std::complex<R>> { using type = R; };
@@ -77,6 +77,7 @@ kr_oracle_opts default_opts() {
   o.shrink = 0.25; o.grow_fast = 8.0; o.grow_mid = 2.0; o.chg_floor = 1e-12;
   o.chg_max = std::numeric_limits<double>::infinity();
   o.it_fast = 3; o.it_mid = 5; o.max_substeps = 4096; o.finalize = 1; o.h_min_rel = 1e-12; o.bail_ratio = 10.0;
+  o.retry = 0; o.retry_h0 = 0.01;
   return o;
 }
 
@@ -393,12 +394,13 @@ bool be_substep(const kr_oracle_network& n, Real Ncal, const double* aux_cell, R
 // ---------------------------------------------------------------------------------------------
 // Steps 1-9 for one cell.  In/out: T, y (double); returns the status bits.
 // ---------------------------------------------------------------------------------------------
+// One attempt at the cell with the options `o`; h0_scale multiplies the first sub-step (1 for the first attempt).
 template <class Real>
-int32_t step_cell(const kr_oracle_network& n, double rho, double& T_io, double* y_io, double dt, const double* aux_cell,
-                  Scratch<Real>& w, Counters& c, double* margin) {
+int32_t step_attempt(const kr_oracle_network& n, const kr_oracle_opts& o, double h0_scale, bool count_failure, double rho,
+                     double& T_io, double* y_io, double dt, const double* aux_cell, Scratch<Real>& w, Counters& c,
+                     double* margin) {
   using std::abs;
-  const int S = n.S, N = n.N, E = n.E;
-  const kr_oracle_opts& o = n.opts;
+  const int S = n.S, N = n.N;
   int32_t st = 0;
   const Real Ncal = Real(rho) / Real(M_U);
 
@@ -431,6 +433,7 @@ int32_t step_cell(const kr_oracle_network& n, double rho, double& T_io, double* 
     for (int s = 0; s < S; ++s) big = std::max(big, Real(abs(w.f[s])) / (Real(abs(w.un[s])) + Real(o.y_floor)));
     if (big > Real(0) && std::isfinite(big)) h = std::min(dtR, Real(o.eta) / big);
   }
+  h = h * Real(h0_scale);
 
   bool failed = false;
   int64_t n_acc = 0, n_rej = 0;
@@ -481,13 +484,30 @@ int32_t step_cell(const kr_oracle_network& n, double rho, double& T_io, double* 
   c.acc += n_acc; c.rej += n_rej;
 
   if (failed) {                                          // R13: revert, never abort
-    c.failed++;
+    if (count_failure) c.failed++;
     return st | ST_FAILED_REVERTED;                      // T_io, y_io untouched
   }
 
   if (o.finalize) st |= finalize_state<Real>(n, w.un.data(), margin);
   for (int s = 0; s < S; ++s) y_io[s] = double(w.un[s]);
   if (n.energy) T_io = double(w.un[S]);
+  return st;
+}
+
+// The retry procedure of PAPER.md:218 (reading R24): a cell whose first attempt fails is tried once more "using identical
+// initial conditions but with reduced initial time step size and enhanced step size control parameters" -- first
+// sub-step x retry_h0, shrink -> shrink^2, grow_fast -> grow_mid, grow_mid -> 1 -- before it is reverted (R13).  The
+// work counters add up over both attempts; the status is the second attempt's with RETRIED set.
+template <class Real>
+int32_t step_cell(const kr_oracle_network& n, double rho, double& T_io, double* y_io, double dt, const double* aux_cell,
+                  Scratch<Real>& w, Counters& c, double* margin) {
+  const kr_oracle_opts& o = n.opts;
+  int32_t st = step_attempt<Real>(n, o, 1.0, !o.retry, rho, T_io, y_io, dt, aux_cell, w, c, margin);
+  if ((st & ST_FAILED_REVERTED) && o.retry) {
+    kr_oracle_opts o2 = o;
+    o2.shrink = o.shrink * o.shrink; o2.grow_fast = o.grow_mid; o2.grow_mid = 1.0;
+    st = step_attempt<Real>(n, o2, o.retry_h0, true, rho, T_io, y_io, dt, aux_cell, w, c, margin) | ST_RETRIED;
+  }
   return st;
 }
 

@@ -41,6 +41,8 @@ typedef struct {
   int32_t it_fast, it_mid, max_substeps, finalize;
   double h_min_rel;                        /* fail when h < h_min_rel * (first sub-step size) */
   double bail_ratio;                       /* early-exit mode: abort the sub-step when e_k > bail_ratio * e_{k-1}, k >= 2 */
+  int32_t retry;                           /* 1: a failed cell is tried once more with tightened control (R24) */
+  double retry_h0;                         /* factor on the first sub-step of the second attempt */
 } kr_oracle_opts;
 
 typedef struct { int64_t n_substeps, n_rejected, n_newton, n_lu, n_rate_evals, n_failed; } kr_oracle_stats;

@@ -35,7 +35,7 @@ class _Opts(C.Structure):
                 ("eta", C.c_double), ("y_floor", C.c_double), ("shrink", C.c_double), ("grow_fast", C.c_double),
                 ("grow_mid", C.c_double), ("chg_floor", C.c_double), ("chg_max", C.c_double),
                 ("it_fast", C.c_int32), ("it_mid", C.c_int32), ("max_substeps", C.c_int32), ("finalize", C.c_int32),
-                ("h_min_rel", C.c_double), ("bail_ratio", C.c_double)]
+                ("h_min_rel", C.c_double), ("bail_ratio", C.c_double), ("retry", C.c_int32), ("retry_h0", C.c_double)]
 
 
 class Stats(C.Structure):
@@ -130,7 +130,8 @@ class OracleNetwork:
     def set_options(self, o) -> None:
         s = _Opts(o.max_newton, o.fixed_newton, o.h0_mode, o.rtol, o.atol_y, o.atol_T, o.neg_tol, o.eta, o.y_floor,
                   o.shrink, o.grow_fast, o.grow_mid, o.chg_floor, o.chg_max, o.it_fast, o.it_mid, o.max_substeps,
-                  getattr(o, "finalize", 1), getattr(o, "h_min_rel", 1e-12), getattr(o, "bail_ratio", 10.0))
+                  getattr(o, "finalize", 1), getattr(o, "h_min_rel", 1e-12), getattr(o, "bail_ratio", 10.0),
+                  getattr(o, "retry", 0), getattr(o, "retry_h0", 0.01))
         rc = load().kr_oracle_set_options(self._h, C.byref(s))
         if rc != 0:
             raise ValueError("kr_oracle_set_options rejected the options")

@@ -20,7 +20,7 @@ LIB_PATH = os.path.join(_HERE, "libkratos_chem.so")
 KR_OK, KR_EINVAL, KR_ENETWORK, KR_ECUDA, KR_EUNSUPPORTED = 0, -1, -2, -3, -4
 KR_FP64, KR_MIXED = 0, 1
 KR_MAP_AUTO, KR_MAP_THREAD, KR_MAP_WARP, KR_MAP_CTA, KR_MAP_THREAD_TABLE, KR_MAP_GROUP_TABLE = 0, 1, 2, 3, 4, 5
-ST_REJECTED_ONCE, ST_CLAMPED_NEG, ST_FP64_FALLBACK, ST_FAILED_REVERTED, ST_T_CLAMPED, ST_NO_RESERVOIR, ST_NEEDS_STAGE3, ST_STAGE3 = 1, 2, 4, 8, 16, 32, 64, 128
+ST_REJECTED_ONCE, ST_CLAMPED_NEG, ST_FP64_FALLBACK, ST_FAILED_REVERTED, ST_T_CLAMPED, ST_NO_RESERVOIR, ST_NEEDS_STAGE3, ST_STAGE3, ST_RETRIED = 1, 2, 4, 8, 16, 32, 64, 128, 256
 
 EXPORTS = [
     "kr_network_create", "kr_network_destroy", "kr_default_opts", "kr_network_set_options",
@@ -55,7 +55,7 @@ class SolverOpts(C.Structure):
                 ("eta", C.c_double), ("y_floor", C.c_double), ("shrink", C.c_double),
                 ("grow_fast", C.c_double), ("grow_mid", C.c_double), ("chg_floor", C.c_double), ("chg_max", C.c_double),
                 ("it_fast", C.c_int32), ("it_mid", C.c_int32), ("max_substeps", C.c_int32), ("finalize", C.c_int32),
-                ("h_min_rel", C.c_double), ("bail_ratio", C.c_double)]
+                ("h_min_rel", C.c_double), ("bail_ratio", C.c_double), ("retry", C.c_int32), ("retry_h0", C.c_double)]
 
 
 class StepStats(C.Structure):

@@ -142,6 +142,8 @@ class SolverOpts:
     h_min_rel: float = 1e-12     # fail when h < h_min_rel * (first sub-step size)
     bail_ratio: float = 10.0     # early-exit mode: abort the sub-step when e_k > bail_ratio * e_{k-1}, k >= 2
     finalize: int = 1            # 0: skip step 9 (used by the conservation pin P4)
+    retry: int = 0               # 1: a failed cell gets a second attempt with tightened control (R24)
+    retry_h0: float = 0.01       # factor on the first sub-step of the second attempt
 
 
 # --------------------------------------------------------------------------

@@ -49,7 +49,7 @@ def test_struct_layouts_match_header(B):
     # kr_network_desc: 3 int32 (+pad), 16 pointers, 2 doubles, 1 int32 (+pad); kr_solver_opts / kr_step_stats
     assert C.sizeof(B.NetworkDesc) == 16 + 16 * 8 + 16 + 8
     assert C.sizeof(B.StepStats) == 48
-    assert C.sizeof(B.SolverOpts) == 16 + 11 * 8 + 16 + 16
+    assert C.sizeof(B.SolverOpts) == 16 + 11 * 8 + 16 + 16 + 16
 
 
 def test_validation_runs_on_the_host_before_any_device_work(B):

@@ -567,3 +567,35 @@ def test_P11_random_states_conserve_and_end_non_negative(oracle_mod):
         if not (st & (32 | 64)):
             assert yo.min() >= 0.0
     assert n3 >= 20                                           # stage 3 was exercised
+
+
+# ---- P12: the retry procedure (reading R24) --------------------------------------------------------------
+def test_P12_retry_second_attempt_with_tightened_control(oracle_mod):
+    """A + A -> A2 with a first sub-step (h = dt, 2 h k N y0 = 1e5) far beyond what K Newton iterations can resolve and a
+    floor three decades below it: the first attempt is rejected five times and gives up.  With retry = 1 the cell is
+    redone from the same input with first sub-step x retry_h0, shrink^2 and slower growth: it then integrates to dt.
+    The result must be the backward-Euler approximation of y0 / (1 + 2 k N y0 t) (above it, within its O(h) error) and
+    conserve a-atoms; both-fail cells are reverted and counted once."""
+    net = H.tiny_network([[1, 2]], [((0, 0), (1,), 1e-10, 0.0, 0.0, 0, -1)])
+    k, Ncal, dt = 1e-10, 1e6, 1e9
+    y0 = np.array([[0.5, 0.25]])
+    cells = H.cells_of(Ncal * H.M_U, 300.0, y0, dt)
+    o = w.SolverOpts(); o.h0_mode = 0; o.max_newton = 6; o.h_min_rel = 1e-3
+    T, y, st, stats, _ = oracle_mod.OracleNetwork(net, o).step(cells)
+    assert st[0] == (8 | 1) and np.array_equal(y, y0) and stats["n_failed"] == 1 and stats["n_rejected"] == 5
+    o.retry = 1
+    T, y, st, stats1, _ = oracle_mod.OracleNetwork(net, o).step(cells)
+    exact = y0[0, 0] / (1.0 + 2.0 * k * Ncal * y0[0, 0] * dt)
+    assert st[0] == (256 | 1), st                                  # RETRIED | REJECTED_ONCE, not FAILED
+    assert exact < y[0, 0] < 1.15 * exact
+    assert abs((y[0, 0] + 2 * y[0, 1]) - (y0[0, 0] + 2 * y0[0, 1])) < 1e-14
+    # counters add up over both attempts: 5 rejections of the first, then 0.01 dt and 0.01 dt / 16 rejected as well
+    assert stats1["n_rejected"] == 5 + 2 and stats1["n_failed"] == 0 and stats1["n_rate_evals"] == 2
+    # a smaller retry_h0 starts below the first acceptable size: fewer rejections in the second attempt
+    o.retry_h0 = 1e-5
+    _, y2, st2, stats2, _ = oracle_mod.OracleNetwork(net, o).step(cells)
+    assert st2[0] == 256 and stats2["n_rejected"] == 5 and exact < y2[0, 0] < 1.15 * exact
+    # both attempts fail: reverted, counted once, flagged FAILED | RETRIED
+    o.retry_h0 = 0.01; o.max_newton = 4
+    T, y3, st3, stats3, _ = oracle_mod.OracleNetwork(net, o).step(cells)
+    assert st3[0] == (8 | 1 | 256) and np.array_equal(y3, y0) and stats3["n_failed"] == 1
