@@ -18,10 +18,10 @@
 // numpy.linalg.solve / Cramer, P6 analytic J vs complex-step, P7 H ionisation-balance quadratic
 // (eq. 35 with eq. 36 coefficients), P8 K=1 equals u_n + h (I-hJ)^-1 f(u_n),
 // P9 adiabatic energy drift O(h^2), P10 long-double witness, P11 post-processing stages 1-3 (exact fractions on a
-// five-species network, row totals, minimal disintegration, charged compounds left alone).
+// five-species network, row totals, minimal disintegration, charged compounds left alone), P12 the retry procedure
+// (R24: closed form of A + A -> A2, counter bookkeeping, both-fail revert).
 // Parity unpinned: the controller constants of step 8 and the choice of Jacobian
-// approximations (dropped dC terms) -- the paper does not publish them.  The two-level retry of PAPER.md:218 is not
-// restated: a cell whose controller gives up is reverted after its first attempt.
+// approximations (dropped dC terms) and the retry parameters of R24 -- the paper does not publish them.
 #include "kr_oracle.h"
 
 #include <algorithm>

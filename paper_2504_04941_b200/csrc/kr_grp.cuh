@@ -477,8 +477,8 @@ __global__ void __launch_bounds__(256) kr_grp_kernel(const KrNetDev n, const KrO
     }
     c_acc += n_acc; c_rej += n_rej;
     if (failed) {                                               // R13: revert
-      c_failed++;
-      if (a.status && G.gl == 0) a.status[cell] = st | KR_DST_FAILED;
+      if (a.fail_list) { if (G.gl == 0) a.fail_list[atomicAdd(a.fail_count, 1ull)] = cell; }   // second attempt
+      else { c_failed++; if (a.status && G.gl == 0) a.status[cell] = st | KR_DST_FAILED; }
       G.sync();
       continue;
     }

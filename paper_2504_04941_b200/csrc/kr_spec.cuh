@@ -524,9 +524,9 @@ kr_spec_kernel(const KrOptsDev o, const KrStepArgs g) {
       }
     }
     if (fail_cell) {                                             // R13: revert (the caller's buffers were never written)
-      c_failed++;
       c_acc += n_acc; c_rej += n_rej;
-      if (g.status) g.status[cell] = st | KR_DST_FAILED;
+      if (g.fail_list) g.fail_list[atomicAdd(g.fail_count, 1ull)] = cell;          // second attempt
+      else { c_failed++; if (g.status) g.status[cell] = st | KR_DST_FAILED; }
       KR_FOR(i, 0, N) u[i] = 1.0; sh.UN(i) = 1.0; KR_END
       phase = KRS_FETCH;
     } else if (cell_done) {                                      // step 9: finalise + layout-out (u == u_n here)

@@ -79,6 +79,7 @@ struct KrOptsDev {
   int max_newton, fixed_newton, h0_mode, it_fast, it_mid, max_substeps, finalize;
   double rtol, atol_y, atol_T, neg_tol, eta, y_floor, shrink, grow_fast, grow_mid, chg_floor, chg_max;
   double h_min_rel, bail_ratio;
+  double h0_scale;       // factor on the first sub-step (1; retry_h0 in the second attempt of the retry procedure)
 };
 
 struct KrStepArgs {
@@ -103,6 +104,10 @@ struct KrStepArgs {
   // isothermal networks, specialised thread-per-cell kernel: rate constants and first sub-step of every cell, written by
   // kr_spec_prelim_kernel as [2R + 1][n_cells] (k_f rows, k_r rows, h0), read by the solve kernel when it loads a cell
   double* prelim;
+  // retry procedure (R24): when non-null, a cell whose controller gives up is appended here (and left
+  // untouched, unflagged, uncounted) for the second attempt instead of being reverted
+  long long* fail_list;
+  unsigned long long* fail_count;
 };
 
 // status bits (mirror of include/kratos_chem.h, kept numeric so that device code needs no host header)
@@ -114,6 +119,7 @@ struct KrStepArgs {
 #define KR_DST_NO_RESERVOIR 32
 #define KR_DST_NEEDS_STAGE3 64
 #define KR_DST_STAGE3 128
+#define KR_DST_RETRIED 256
 
 #define KR_DF_REV 1
 #define KR_DF_TB 2

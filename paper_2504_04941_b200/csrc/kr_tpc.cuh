@@ -340,9 +340,9 @@ __global__ void __launch_bounds__(KR_TPC_BD) kr_tpc_kernel(const KrNetDev n, con
         }
       }
       if (fail_cell) {                                           // R13: revert (global T, y untouched)
-        c_failed++;
         c_acc += n_acc; c_rej += n_rej;
-        if (a.status) a.status[cell] = st | KR_DST_FAILED;
+        if (a.fail_list) a.fail_list[atomicAdd(a.fail_count, 1ull)] = cell;        // second attempt
+        else { c_failed++; if (a.status) a.status[cell] = st | KR_DST_FAILED; }
         phase = KR_PH_FETCH;
       } else if (cell_done) {                                    // step 9: finalise + layout-out
         c_acc += n_acc; c_rej += n_rej;

@@ -729,6 +729,7 @@ kr_wpc_kernel(const KrNetDev n, const KrOptsDev o, const KrStepArgs a) {
     // The first pass of a cell through the evaluation below is its preliminary evaluation: rate constants of an
     // isothermal cell, f(u_in) for the first sub-step (step 1, h0_mode 1).  One call site keeps the kernel small.
     bool prelim = (o.h0_mode == 1) || !ENERGY || (a.cost_out != nullptr);
+    if (!prelim) { h = h * o.h0_scale; h_floor = o.h_min_rel * fmin(h, a.dt); }
 
     // ---- sub-step loop (steps 6-8) -------------------------------------------------------------------------------
     bool failed = false, handoff = false;
@@ -759,6 +760,7 @@ kr_wpc_kernel(const KrNetDev n, const KrOptsDev o, const KrStepArgs a) {
             big = G.max(big);
             if (big > 0.0 && finite(big)) h = fmin(a.dt, o.eta / big);
           }
+          h = h * o.h0_scale;
           h_floor = o.h_min_rel * fmin(h, a.dt);
           prelim = false; was_prelim = true;
           break;
@@ -856,8 +858,8 @@ kr_wpc_kernel(const KrNetDev n, const KrOptsDev o, const KrStepArgs a) {
     }
     c_acc += n_acc; c_rej += n_rej;
     if (failed) {                                                 // R13: revert (the caller's buffers were never written)
-      c_failed++;
-      if (a.status && G.gl == 0) a.status[cell] = st | KR_DST_FAILED;
+      if (a.fail_list) { if (G.gl == 0) a.fail_list[atomicAdd(a.fail_count, 1ull)] = cell; }   // second attempt
+      else { c_failed++; if (a.status && G.gl == 0) a.status[cell] = st | KR_DST_FAILED; }
       G.sync();
       continue;
     }

@@ -318,6 +318,36 @@ def test_post_processing_stage_3(B, oracle_mod, idx, mapping, tpc):
     assert (np.abs((yg - y) @ comp.T.astype(np.float64)) / tot).max() <= 1e-14
 
 
+@pytest.mark.parametrize("idx,n,mapping,tpc,mode", [(1, 400, None, 0, 0), (2, 600, None, 0, 0), (3, 120, None, 0, 0), (1, 200, 4, 1, 0),
+                                                     (3, 90, 5, 32, 0)])
+def test_retry_procedure(B, oracle_mod, idx, n, mapping, tpc, mode):
+    """PAPER.md:218 / R24: with h = dt first, six Newton iterations and a floor three decades below the first sub-step many
+    cells give up in their first attempt; with retry = 1 they are listed and redone from their input by one more launch
+    (first sub-step x 0.01, shrink^2, slower growth).  Status (RETRIED, FAILED), results and counters against the oracle."""
+    net, cells, opts = w.make_config(idx, n)
+    opts.h0_mode = 0; opts.max_newton = 6; opts.h_min_rel = 1e-3; opts.retry = 1
+    ref = P.oracle_reference(oracle_mod, net, cells, opts)
+    retried = (ref["status"] & 256) != 0
+    assert retried.sum() >= 10 and ((ref["status"][retried] & 8) == 0).sum() >= 5
+    T, y, st, stats, gn = run_gpu(B, net, cells, opts, mode=mode, mapping=mapping, tpc=tpc)
+    out = P.compare(net, ref, T, y, st & ~B.ST_FP64_FALLBACK, tol=MIXED_TOL if mode else P.TOL, allow_path_flips=0.03)
+    m = ref["comparable"]
+    assert ((st[m] & 256) == (ref["status"][m] & 256)).all() and ((st[m] & 8) == (ref["status"][m] & 8)).all()
+    assert stats["n_failed"] == int(((st & 8) != 0).sum())
+    if mode == 0 and out["n_comparable"] == out["n"]:
+        # same sub-steps, rejections and failures; the Newton iterations of REJECTED sub-steps may differ by a few (iterates
+        # started at h = dt overflow, and where the non-finite value is first seen differs between the implementations)
+        for key in ("n_substeps", "n_rejected", "n_failed"):
+            assert stats[key] == ref["stats"][key], key
+        assert abs(stats["n_newton"] - ref["stats"]["n_newton"]) <= 1e-3 * ref["stats"]["n_newton"]
+    rev = (st & 8) != 0
+    np.testing.assert_array_equal(y[rev], cells.y[rev])          # failed twice: reverted to the input
+    # without the option the same cells are reverted after the first attempt
+    opts.retry = 0
+    T0, y0, st0, stats0, _ = run_gpu(B, net, cells, opts, mode=mode, mapping=mapping, tpc=tpc)
+    assert ((st0 & 256) == 0).all() and ((st0 & 8) != 0).sum() >= retried[m].sum() * 0.9
+
+
 def test_argument_errors(B):
     import torch
     net, cells, opts = w.make_config(2, 8)
