@@ -361,6 +361,11 @@ def test_argument_errors(B):
         gn.thermochem_step_ex(8, rho, T, y, cells.dt, 7, aux=aux)
     with pytest.raises(B.KrError):            # dt
         gn.thermochem_step_ex(8, rho, T, y, -1.0, 0, aux=aux)
+    o = w.default_opts(2); o.retry = 1
+    gr = B.Network(net, o)
+    with pytest.raises(B.KrError) as e:       # the retry procedure is an fp64 feature
+        gr.thermochem_step_ex(8, rho, T, y, cells.dt, B.KR_MIXED, aux=aux)
+    assert e.value.code == B.KR_EUNSUPPORTED
     with pytest.raises(B.KrError) as e:       # thread-per-cell cannot hold N = 64
         B.Network(w.make_network(4)).set_mapping(B.KR_MAP_THREAD)
     assert e.value.code == B.KR_EUNSUPPORTED
