@@ -146,6 +146,21 @@ def test_stiffest_first_scheduling_changes_nothing(B, monkeypatch):
     assert st1 == st0
 
 
+def test_retry_with_stiffest_first_scheduling(B, monkeypatch):
+    """The retry pass behind a list-driven first launch (several waves -> cost pass + sort): every cell is written exactly
+    once, and the result equals the index-order run bit for bit."""
+    net, cells, opts = w.make_config(3, 9000)
+    opts.h0_mode = 0; opts.max_newton = 6; opts.h_min_rel = 1e-3; opts.retry = 1
+    T1, y1, s1, st1, g1 = run_gpu(B, net, cells, opts)
+    assert (s1 >= 0).all() and ((s1 & 256) != 0).sum() > 1000          # run_gpu pre-fills the status with -1
+    assert g1.last_launch_count() == 10
+    monkeypatch.setenv("KR_NO_LPT", "1")
+    T0, y0, s0, st0, g0 = run_gpu(B, net, cells, opts)
+    np.testing.assert_array_equal(y1, y0)
+    np.testing.assert_array_equal(s1, s0)
+    assert st1 == st0 and g0.last_launch_count() == 2
+
+
 def test_mixed_fallback_cells_equal_the_fp64_run(B):
     """A cell the fp32 factorisation cannot resolve is redone from its input by the fp64 kernel: its result must be the
     fp64 mode's result bit for bit, with KR_ST_FP64_FALLBACK set and nothing else changed."""
