@@ -98,8 +98,7 @@ typedef struct {
   double h_min_rel;     /* fail when h < h_min_rel * (first sub-step size) */
   double bail_ratio;    /* early-exit mode: abort the sub-step when e_k > bail_ratio * e_{k-1}, k >= 2 */
   int32_t retry;        /* 1: a cell whose first attempt fails is redone from its input with tightened control before it is
-                         * reverted (R24): one more launch on the listed cells.  Default 0; KR_FP64 only
-                         * (KR_EUNSUPPORTED with KR_MIXED). */
+                         * reverted (R24): one more launch (fp64) on the listed cells.  Default 0. */
   double retry_h0;      /* factor on the first sub-step of the second attempt (default 0.01) */
 } kr_solver_opts;
 

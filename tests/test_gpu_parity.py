@@ -161,6 +161,27 @@ def test_retry_with_stiffest_first_scheduling(B, monkeypatch):
     assert st1 == st0 and g0.last_launch_count() == 2
 
 
+def test_one_handle_serves_both_precision_modes_and_sizes(B):
+    """Workspace reuse on one handle: fp64 with stiffest-first scheduling, then mixed (allocates its retry list), then fp64
+    again with a larger batch -- the cached buffers of one mode must survive the other (a mis-placed cudaFree once did not)."""
+    import torch
+    net, cells, opts = w.make_config(3, 9000)
+    gn = B.Network(net, opts)
+    outs = []
+    for mode, n in ((0, 7000), (1, 7000), (0, 9000), (1, 9000), (0, 7000)):
+        sub = cells.take(slice(0, n))
+        rho = torch.tensor(sub.rho, device="cuda"); T = torch.tensor(sub.T, device="cuda"); y = torch.tensor(sub.y, device="cuda")
+        aux = torch.tensor(sub.aux, device="cuda")
+        st = torch.full((n,), -1, dtype=torch.int32, device="cuda")
+        gn.thermochem_step_ex(n, rho, T, y, sub.dt, mode, aux=aux, status=st)
+        torch.cuda.synchronize()
+        assert (st >= 0).all()
+        outs.append(y.cpu().numpy())
+    np.testing.assert_array_equal(outs[0], outs[4])                  # same call, same bits, before and after the others
+    np.testing.assert_array_equal(outs[0], outs[2][:7000])
+    assert P.rel_err(outs[1], outs[0]).max() < 1e-6 and P.rel_err(outs[3], outs[2]).max() < 1e-6
+
+
 def test_mixed_fallback_cells_equal_the_fp64_run(B):
     """A cell the fp32 factorisation cannot resolve is redone from its input by the fp64 kernel: its result must be the
     fp64 mode's result bit for bit, with KR_ST_FP64_FALLBACK set and nothing else changed."""
@@ -333,8 +354,8 @@ def test_post_processing_stage_3(B, oracle_mod, idx, mapping, tpc):
     assert (np.abs((yg - y) @ comp.T.astype(np.float64)) / tot).max() <= 1e-14
 
 
-@pytest.mark.parametrize("idx,n,mapping,tpc,mode", [(1, 400, None, 0, 0), (2, 600, None, 0, 0), (3, 120, None, 0, 0), (1, 200, 4, 1, 0),
-                                                     (3, 90, 5, 32, 0)])
+@pytest.mark.parametrize("idx,n,mapping,tpc,mode", [(1, 400, None, 0, 0), (2, 600, None, 0, 0), (3, 120, None, 0, 0), (3, 120, None, 0, 1),
+                                                     (1, 200, 4, 1, 0), (3, 90, 5, 32, 0)])
 def test_retry_procedure(B, oracle_mod, idx, n, mapping, tpc, mode):
     """PAPER.md:218 / R24: with h = dt first, six Newton iterations and a floor three decades below the first sub-step many
     cells give up in their first attempt; with retry = 1 they are listed and redone from their input by one more launch
@@ -376,11 +397,6 @@ def test_argument_errors(B):
         gn.thermochem_step_ex(8, rho, T, y, cells.dt, 7, aux=aux)
     with pytest.raises(B.KrError):            # dt
         gn.thermochem_step_ex(8, rho, T, y, -1.0, 0, aux=aux)
-    o = w.default_opts(2); o.retry = 1
-    gr = B.Network(net, o)
-    with pytest.raises(B.KrError) as e:       # the retry procedure is an fp64 feature
-        gr.thermochem_step_ex(8, rho, T, y, cells.dt, B.KR_MIXED, aux=aux)
-    assert e.value.code == B.KR_EUNSUPPORTED
     with pytest.raises(B.KrError) as e:       # thread-per-cell cannot hold N = 64
         B.Network(w.make_network(4)).set_mapping(B.KR_MAP_THREAD)
     assert e.value.code == B.KR_EUNSUPPORTED
