@@ -155,6 +155,7 @@ def main() -> None:
     ap.add_argument("--cells", type=int, default=0, help="override the cell count (testing only)")
     ap.add_argument("--mapping", type=int, default=0, help="override the per-cell mapping (KR_MAP_*; mapping study only)")
     ap.add_argument("--threads-per-cell", type=int, default=0)
+    ap.add_argument("--retry", action="store_true", help="enable the retry procedure (PAPER.md:218; study only, default options have it off)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -187,6 +188,8 @@ def main() -> None:
     # no data-path collective)
     cells = w.make_cells(idx, net, n_cells, seed=w.BASE_SEED + 1000 + idx + 7919 * rank)
     opts = w.default_opts(idx, fixed_newton=0)
+    if args.retry:
+        opts.retry = 1
     gn = B.Network(net, opts)
     if args.mapping:
         gn.set_mapping(args.mapping, args.threads_per_cell)
@@ -291,7 +294,7 @@ def main() -> None:
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64" if mode == B.KR_FP64 else "f32+f64", "data": "synthetic",
             "config": {"workload": w.CONFIG_NAMES[idx], "cells_per_gpu": n_cells, "S": net.n_species, "R": net.n_reac,
-                       "N": net.n_unknowns, "dt": cells.dt, "newton": "early-exit, K<=8", "precision_mode": args.mode,
+                       "N": net.n_unknowns, "dt": cells.dt, "newton": "early-exit, K<=8", "precision_mode": args.mode, "retry": int(bool(args.retry)),
                        "mapping": {1: "thread-per-cell", 2: "warp-per-cell", 3: "cta-per-cell", 4: "thread-per-cell (table)",
                                    5: "group-per-cell (table)"}[info["mapping"]],
                        "kernel": gn.kernel_desc(),
