@@ -154,7 +154,10 @@ int kr_thermochem_step_ex(kr_network *net, int64_t n_cells, const double *rho, d
 
 /* Host-buffer convenience used for the end-to-end measurement: same arguments as kr_thermochem_step_ex
  * but rho, T, y, aux, status are HOST pointers; the call stages them through device buffers cached on
- * the handle (host->device copies, the step, device->host copies of T, y, status) and synchronises. */
+ * the handle (host->device copies, the step, device->host copies of T, y, status) and synchronises.  Batches of
+ * 2^19 cells or more without stats are cut into 4 chunks and pipelined (copy-in, step, copy-out on separate
+ * streams) once an unchunked call on the handle has shown the copies to exceed 30 % of the step; results are identical
+ * to the unchunked call.  Host buffers should be pinned for the copies to overlap. */
 int kr_thermochem_step_host(kr_network *net, int64_t n_cells, const double *rho, double *T, double *y, double dt,
                             int precision_mode, const double *aux, int32_t n_aux, int32_t *status,
                             kr_step_stats *stats);
