@@ -2,7 +2,7 @@
 // N <= 64 in mixed precision).  Compiled at kr_network_create (NVRTC, sm_100a) with the sizes of the network
 // as macros, so every register tile is exactly as large as the network needs:
 //   KRW_N KRW_S KRW_R KRW_E KRW_ENERGY KRW_ANY_REV KRW_ANY_TB KRW_ANY_QEXT KRW_NAUX    the network
-//   KRW_W      warps per cell (1 or 2)         KRW_TR  row groups inside a warp (4 or 8; TC = 32 / TR)
+//   KRW_W      warps per cell (1 or 2)         KRW_TR  row groups inside a warp (4, 8 or 16; TC = 32 / TR)
 //   KRW_RB     rows per thread (TR RB >= N)    KRW_CB  columns per thread (TC W CB >= N + 1)
 //   KRW_MIXED  0: fp64 throughout   1: fp32 matrix + elimination, fp64 residuals, iterative refinement (R15)
 //   KRW_CPB    cells per block                 KRW_MIN_BLOCKS  launch bound
