@@ -1,25 +1,37 @@
 #!/usr/bin/env python
 """bench.py -- cell-updates/s of one implicit chemistry step (kr_thermochem_step) on B200.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1] [--mode fp64|mixed] [--impl reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--mode fp64|mixed] [--scaling weak|strong]
+                  [--impl reference]
 
 A "step" is one pass of the whole hot path (layout-in, thermo, rate constants, rates of progress,
 Jacobian, LU + substitution, Newton loop, sub-step controller, finalise, layout-out: DESIGN.md a1-a9)
-over every cell of the workload, i.e. one kr_thermochem_step call.  Default workload: BASELINE.json
-configs[1] (combustion-like, S = 9, R = 21, N = 10, 2^20 cells, fp64, early-exit Newton), seeded synthetic.
+over every cell of the workload, i.e. one kr_thermochem_step call.
 
-One JSON line is printed by rank 0.  ``value`` is device-timed (CUDA events around each call, state
-restored and L2 flushed before each timed call, outside the events); ``e2e`` goes through
-kr_thermochem_step_host with pinned HOST buffers (copies inside the timed region).  ``roofline`` is the
-algorithmic FP64 work (paper_2504_04941_b200/flops.py, from the solver's own counters) over the kernel's
-event-timed duration, against the FP64 FMA peak measured in this run by kr_measure_fp64_peak.
-``--impl reference`` times the CPU oracle (oracle/, test infrastructure) on a bounded sample.
+ONE JSON line is printed by rank 0.  Its top-level fields are the headline workload -- BASELINE.json configs[1]
+(combustion-like, S = 9, R = 21, N = 10, 2^20 cells, fp64, early-exit Newton; the configuration the metric is quoted on
+that fits one GPU) -- and, when no --config is given, ``"configs"`` lists the same measurements for ALL five BASELINE
+configs in fp64 and for configs 3 and 4 in mixed precision (BASELINE.json: "cell-updates/s ... (fp64, mixed) and % of
+FP64/HBM roofline", per config).  ``--config C [--mode M]`` measures that one workload only.
+
+``value`` is device-timed (CUDA events around each call on the stream the library launches on, state restored and L2
+flushed before each timed call, outside the events); ``e2e`` goes through kr_thermochem_step_host with pinned HOST
+buffers (copies inside the timed region).  ``roofline`` is the algorithmic FP64 work (paper_2504_04941_b200/flops.py,
+from the solver's own counters) over the event-timed duration, against the FP64 FMA peak measured in this run by
+kr_measure_fp64_peak.  ``cpu_baseline`` / ``--impl reference`` time the CPU oracle (oracle/, test infrastructure) on a
+bounded sample, on all host cores and on one thread.
+
+``--gpus N`` with N > 1 and no torchrun environment starts N ranks itself (one process per GPU, NCCL for the counter and
+time reductions only: cells are independent).  ``--scaling weak`` (default) gives every rank a
+full-size, differently seeded batch; ``--scaling strong`` shards ONE full-size batch block-cyclically over the ranks
+(paper_2504_04941_b200/parallel.py, shard_indices).
 """
 from __future__ import annotations
 
 import argparse
 import json
 import os
+import socket
 import sys
 import threading
 import time
@@ -35,11 +47,12 @@ from paper_2504_04941_b200 import workloads as w      # noqa: E402
 
 METRIC = "cell-updates/s for one implicit chem step"
 UNIT = "cell-updates/s"
-
-# DRAM traffic of the step kernel per cell-update, from the ncu --set full captures summarised under profiles/
-# (dram__bytes_read.sum + dram__bytes_write.sum of one launch / cells of that launch).  It is BELOW the algorithmic
-# bytes because the results of the last cells are still in the 126 MB L2 when the kernel ends.
-NCU_DRAM_BYTES_PER_CELL = {("c1", "fp64"): 130.2, ("c3", "fp64"): 285.8}
+HEADLINE = 1
+# every (config, precision) BASELINE.json asks for
+ALL_RUNS = [(0, "fp64"), (1, "fp64"), (2, "fp64"), (3, "fp64"), (4, "fp64"), (3, "mixed"), (4, "mixed")]
+MAPPING_NAMES = {1: "thread-per-cell", 2: "warp-per-cell", 3: "cta-per-cell", 4: "thread-per-cell (table)", 5: "group-per-cell (table)"}
+TRAFFIC_NOTE = ("null: DRAM bytes are not measurable inside the run; the ncu --set full captures of the step kernels "
+                "(dram__bytes_read.sum + dram__bytes_write.sum per launch) are under profiles/, each with its command")
 
 
 class ClockSampler(threading.Thread):
@@ -91,11 +104,16 @@ class ClockSampler(threading.Thread):
                 "samples": len(self.samples)}
 
 
-def oracle_sample_rate(net, cells, opts, target_seconds: float, cores: int):
-    """Time the oracle as it stands on a bounded prefix of the workload; returns (cells/s, n_sample, seconds)."""
+def _oracle():
     from oracle import build as obuild
     obuild.build_oracle()
     from oracle import oracle as O
+    return O
+
+
+def oracle_rates(net, cells, opts, target_seconds: float, cores: int) -> dict:
+    """The oracle as it stands on a bounded prefix of the workload: all host cores, then one thread."""
+    O = _oracle()
     on = O.OracleNetwork(net, opts)
     n = min(cells.n_cells, 64 * cores)
     t0 = time.perf_counter()
@@ -105,18 +123,22 @@ def oracle_sample_rate(net, cells, opts, target_seconds: float, cores: int):
     t0 = time.perf_counter()
     on.step(cells.take(slice(0, n2)), n_threads=cores)
     t2 = time.perf_counter() - t0
-    return n2 / t2, n2, t2
+    rate_all = n2 / t2
+    n1 = int(max(8, min(n2, rate_all / cores * 0.35 * target_seconds)))      # ~a third of the budget on one thread
+    t0 = time.perf_counter()
+    on.step(cells.take(slice(0, n1)), n_threads=1)
+    t1 = time.perf_counter() - t0
+    return {"value": rate_all, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"first {n2} cells of the same seeded workload, {t2:.1f} s, {cores} threads",
+            "one_thread": {"value": n1 / t1, "unit": UNIT, "cores": 1, "sample": f"first {n1} cells, {t1:.1f} s"}}
 
 
-def run_reference(args, rank: int, world: int) -> None:
+def run_reference(args) -> None:
     """--impl reference: the CPU oracle on the host cores, bounded sample per step (rank 0 only)."""
-    if rank != 0:
-        return
+    idx = HEADLINE if args.config is None else args.config
     cores = os.cpu_count() or 1
-    net, cells, opts = w.make_config(args.config, min(w.FULL_CELLS[args.config], 1 << 16))
-    from oracle import build as obuild
-    obuild.build_oracle()
-    from oracle import oracle as O
+    net, cells, opts = w.make_config(idx, min(w.FULL_CELLS[idx], 1 << 16))
+    O = _oracle()
     on = O.OracleNetwork(net, opts)
     n = min(cells.n_cells, 64 * cores)
     t0 = time.perf_counter()
@@ -133,9 +155,9 @@ def run_reference(args, rank: int, world: int) -> None:
     dt = time.perf_counter() - t0
     value = n_s * args.steps / dt
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+            "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": args.scaling,
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": w.CONFIG_NAMES[args.config], "cells_per_step": n_s, "newton": "early-exit",
+            "config": {"workload": w.CONFIG_NAMES[idx], "cells_per_step": n_s, "newton": "early-exit",
                        "note": "CPU oracle (oracle/kr_oracle.cpp, -O2, std::thread over disjoint cell ranges)"},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
                              "sample": f"first {n_s} cells of the seeded workload per step"},
@@ -144,49 +166,24 @@ def run_reference(args, rank: int, world: int) -> None:
     print(json.dumps(line), flush=True)
 
 
-def main() -> None:
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
-    ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=1)
-    ap.add_argument("--mode", default="fp64", choices=["fp64", "mixed"])
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--cells", type=int, default=0, help="override the cell count (testing only)")
-    ap.add_argument("--mapping", type=int, default=0, help="override the per-cell mapping (KR_MAP_*; mapping study only)")
-    ap.add_argument("--threads-per-cell", type=int, default=0)
-    ap.add_argument("--retry", action="store_true", help="enable the retry procedure (PAPER.md:218; study only, default options have it off)")
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-e2e", action="store_true")
-    args = ap.parse_args()
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    if args.impl == "reference":
-        run_reference(args, rank, world)
-        return
-
+def bench_one(idx: int, mode_name: str, args, ctx) -> dict:
+    """Measure one (config, precision) on this rank's GPU; returns the result dict (rank 0's is printed)."""
     import torch
     import torch.distributed as dist
     from paper_2504_04941_b200 import binding as B
     from paper_2504_04941_b200 import parallel as par
 
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: the library has no CPU path")
-    torch.cuda.set_device(local_rank)
-    dev = torch.device("cuda", local_rank)
-    if world > 1:
-        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", device_id=dev)
-    B.load()
-
-    idx = args.config
-    mode = B.KR_FP64 if args.mode == "fp64" else B.KR_MIXED
-    n_cells = args.cells or w.FULL_CELLS[idx]
+    rank, world, dev = ctx["rank"], ctx["world"], ctx["dev"]
+    mode = B.KR_FP64 if mode_name == "fp64" else B.KR_MIXED
+    full = args.cells or w.FULL_CELLS[idx]
     net = w.make_network(idx)
-    # weak scaling: every rank integrates a full-size, differently seeded batch (cells are independent:
-    # no data-path collective)
-    cells = w.make_cells(idx, net, n_cells, seed=w.BASE_SEED + 1000 + idx + 7919 * rank)
+    if args.scaling == "strong" and world > 1:
+        # ONE full-size batch (the rank-0 seed), sharded block-cyclically: every rank draws the same batch and keeps its share
+        cells = par.shard_cells(w.make_cells(idx, net, full, seed=w.BASE_SEED + 1000 + idx), rank, world)
+    else:
+        # weak scaling: every rank integrates a full-size, differently seeded batch (no data-path collective)
+        cells = w.make_cells(idx, net, full, seed=w.BASE_SEED + 1000 + idx + 7919 * rank)
+    n_cells = cells.n_cells
     opts = w.default_opts(idx, fixed_newton=0)
     if args.retry:
         opts.retry = 1
@@ -202,7 +199,7 @@ def main() -> None:
     aux = None if cells.aux is None else torch.tensor(cells.aux, device=dev)
     T = T0.clone(); y = y0.clone()
     status = torch.zeros(n_cells, dtype=torch.int32, device=dev)
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)       # > 126 MB L2
+    flush = ctx["flush"]
 
     def restore():
         T.copy_(T0); y.copy_(y0)
@@ -211,13 +208,13 @@ def main() -> None:
     def step(want_stats=False):
         return gn.thermochem_step_ex(n_cells, rho, T, y, cells.dt, mode, aux=aux, status=status, want_stats=want_stats)
 
-    peak_tf = B.measure_fp64_peak(8192)
-    for _ in range(max(args.warmup, 3)):
+    warm = max(args.warmup, 3)
+    for _ in range(warm):
         restore(); step()
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
-    sampler = ClockSampler(local_rank)
+    sampler = ClockSampler(ctx["local_rank"])
     sampler.start()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     torch.cuda.synchronize()
@@ -248,12 +245,13 @@ def main() -> None:
     if mode == B.KR_MIXED:
         ms = gn.last_mixed_stats()
         mixed_stats = {"refinements_per_newton": ms["n_refine"] / max(stats["n_newton"], 1),
-                       "fp64_fallback_cell_fraction": ms["n_fp64_cells"] / n_cells,
-                       "fp64_kernel": "register-tile fp64 kernel on the listed cells (second launch)"}
+                       "fp64_fallback_cell_fraction": ms["n_fp64_cells"] / max(n_cells, 1),
+                       "fp64_kernel": "fp64 warp-per-cell kernel on the listed cells (second launch)"}
     flops_step = F.step_flops(net, stats)
-    kern_ms = float(np.mean(ms_each))                     # this rank's kernel: one launch per step
+    kern_ms = float(np.mean(ms_each))                     # this rank's step
     achieved_tf = flops_step / (kern_ms * 1e-3) / 1e12
-    bytes_step = F.step_bytes(net, n_cells, 0 if cells.aux is None else cells.aux.shape[0])
+    n_aux = 0 if cells.aux is None else cells.aux.shape[0]
+    bytes_step = F.step_bytes(net, n_cells, n_aux)
 
     # end to end: pinned host buffers through kr_thermochem_step_host
     e2e = None
@@ -274,7 +272,6 @@ def main() -> None:
             if k > 0:
                 t_e2e += time.perf_counter() - t0
         t_e2e = par.max_over_ranks(t_e2e)
-        n_aux = 0 if cells.aux is None else cells.aux.shape[0]
         h2d = n_cells * 8 * (2 + net.n_species + n_aux)
         d2h = n_cells * (8 * (net.n_species + net.energy_equation) + 4)
         e2e = {"value": cells_total * n_e2e / t_e2e, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
@@ -282,40 +279,133 @@ def main() -> None:
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        cores = os.cpu_count() or 1
-        rate, n_s, secs = oracle_sample_rate(net, cells, opts, 12.0, cores)
-        cpu = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
-               "sample": f"first {n_s} cells of the same seeded workload, {secs:.1f} s, {cores} threads"}
+        cpu = oracle_rates(net, cells, opts, args.cpu_seconds, os.cpu_count() or 1)
 
+    info = gn.info()
+    peak_tf = ctx["peak_tf"]
+    notes = []
+    if n_cells <= 65536:
+        notes.append("launch bound: two kernel launches per step on 4 096 cells (a correctness config)")
+    if idx in (3, 4) or info["mapping"] in (2, 3):
+        notes.append("the timed step includes the stiffest-first scheduling: cost pass, iota and a CUB radix sort (library kernels, ~0.3 % of the step)")
+    if idx == 3:
+        notes.append("workload deviation D2 (DESIGN.md section 4): the 140 two-body reactions are one-way, so this config has no reverse-rate exponentials")
+    if idx == 4:
+        notes.append("workload deviation D2 (DESIGN.md section 4): associations use A x 1e-6 and bond-like formation enthalpies")
+    return {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": warm,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": args.scaling, "vs_baseline": None,
+        "dtype": "f64" if mode == B.KR_FP64 else "f32+f64", "data": "synthetic",
+        "config": {"workload": w.CONFIG_NAMES[idx], "cells_per_gpu": n_cells, "S": net.n_species, "R": net.n_reac,
+                   "N": net.n_unknowns, "dt": cells.dt, "newton": "early-exit, K<=8", "precision_mode": mode_name,
+                   "retry": int(bool(args.retry)), "mapping": MAPPING_NAMES[info["mapping"]], "kernel": gn.kernel_desc(),
+                   "threads_per_cell": info["threads_per_cell"], "smem_bytes_per_block": info["smem_bytes"],
+                   "l2": "state restored from a pristine copy and a 256 MiB buffer written before every timed call",
+                   "parallelism": f"cells sharded ({args.scaling} scaling), {world} rank(s), no data-path collective",
+                   "notes": notes},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
+        "roofline": {"bound": "alu", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
+                     "frac": achieved_tf / peak_tf, "traffic": None, "traffic_note": TRAFFIC_NOTE,
+                     "peak_source": "FP64 FMA peak measured in this run (kr_measure_fp64_peak); nominal 148 SM x 64 FMA/clk x 2 x 1.965 GHz = 37.2",
+                     "flops_per_launch": flops_step, "kernel_ms": kern_ms,
+                     "hbm_bytes_per_launch": bytes_step, "hbm_gbs": bytes_step / (kern_ms * 1e-3) / 1e9},
+        "cpu_baseline": cpu,
+        "solver": {k: v / max(n_cells, 1) for k, v in stats.items()}, "n_failed": n_failed, "wall_s_timed_region": wall,
+        "mixed": mixed_stats,
+    }
+
+
+def worker(args, rank: int, local_rank: int, world: int) -> None:
+    import torch
+    import torch.distributed as dist
+    from paper_2504_04941_b200 import binding as B
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the library has no CPU path")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=dev)
+    B.load()
+    ctx = dict(rank=rank, local_rank=local_rank, world=world, dev=dev,
+               flush=torch.empty(256 << 20, dtype=torch.uint8, device=dev),       # > 126 MB L2
+               peak_tf=B.measure_fp64_peak(8192))
+    if args.config is not None:
+        runs = [(args.config, args.mode)]
+    elif world > 1 and not args.all_configs:
+        runs = [(HEADLINE, "fp64")]              # scaling runs time the headline workload; --all-configs for the rest
+    else:
+        runs = ALL_RUNS
+    results = []
+    for idx, mode_name in runs:
+        results.append(bench_one(idx, mode_name, args, ctx))
+        torch.cuda.empty_cache()
     if rank == 0:
-        info = gn.info()
-        line = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64" if mode == B.KR_FP64 else "f32+f64", "data": "synthetic",
-            "config": {"workload": w.CONFIG_NAMES[idx], "cells_per_gpu": n_cells, "S": net.n_species, "R": net.n_reac,
-                       "N": net.n_unknowns, "dt": cells.dt, "newton": "early-exit, K<=8", "precision_mode": args.mode, "retry": int(bool(args.retry)),
-                       "mapping": {1: "thread-per-cell", 2: "warp-per-cell", 3: "cta-per-cell", 4: "thread-per-cell (table)",
-                                   5: "group-per-cell (table)"}[info["mapping"]],
-                       "kernel": gn.kernel_desc(),
-                       "threads_per_cell": info["threads_per_cell"], "smem_bytes_per_block": info["smem_bytes"],
-                       "l2": "state restored from a pristine copy and a 256 MiB buffer written before every timed call",
-                       "parallelism": f"cells sharded, {world} rank(s), no data-path collective"},
-            "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
-            "roofline": {"bound": "alu", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
-                         "frac": achieved_tf / peak_tf,
-                         "traffic": (NCU_DRAM_BYTES_PER_CELL[(f"c{idx}", args.mode)] * n_cells
-                                     if (f"c{idx}", args.mode) in NCU_DRAM_BYTES_PER_CELL else None),
-                         "peak_source": "FP64 FMA peak measured in this run (kr_measure_fp64_peak); nominal 148 SM x 64 FMA/clk x 2 x 1.965 GHz = 37.2",
-                         "flops_per_launch": flops_step, "kernel_ms": kern_ms,
-                         "hbm_bytes_per_launch": bytes_step, "hbm_gbs": bytes_step / (kern_ms * 1e-3) / 1e9},
-            "cpu_baseline": cpu,
-            "solver": {k: v / n_cells for k, v in stats.items()}, "n_failed": n_failed, "wall_s_timed_region": wall,
-            "mixed": mixed_stats,
-        }
+        head = next((r for r, (i, m) in zip(results, runs) if i == HEADLINE and m == "fp64"), results[0])
+        line = dict(head)
+        if len(results) > 1:
+            line["config"] = dict(head["config"])
+            line["config"]["headline"] = ("BASELINE.json configs[1]: the configuration the base contract names for N = 1; every other "
+                                          "config and both precisions are measured in the same run under \"configs\" (lowest "
+                                          "roofline fraction at S >= 9: see there)")
+            line["configs"] = [{"workload": r["config"]["workload"], "dtype": r["dtype"], "value": r["value"],
+                                "ms_per_step": r["ms_per_step"], "roofline": r["roofline"], "e2e": r["e2e"],
+                                "cpu_baseline": r["cpu_baseline"], "n_failed": r["n_failed"], "solver": r["solver"],
+                                "gpu_launches": r["gpu_launches"], "clocks": r["clocks"], "mixed": r["mixed"],
+                                "kernel": r["config"]["kernel"], "cells_per_gpu": r["config"]["cells_per_gpu"],
+                                "notes": r["config"]["notes"]} for r in results]
+            line["gpu_launches"] = int(sum(r["gpu_launches"] for r in results))
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
+
+
+def _spawn_entry(local_rank: int, args, world: int, port: int) -> None:
+    os.environ.update(RANK=str(local_rank), LOCAL_RANK=str(local_rank), WORLD_SIZE=str(world),
+                      MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    worker(args, local_rank, local_rank, world)
+
+
+def main() -> None:
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=None, help="measure this BASELINE config only (default: all of them, headline = 1)")
+    ap.add_argument("--mode", default="fp64", choices=["fp64", "mixed"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"])
+    ap.add_argument("--all-configs", action="store_true", help="with --gpus N > 1: measure every config, not only the headline")
+    ap.add_argument("--cells", type=int, default=0, help="override the cell count (testing only)")
+    ap.add_argument("--mapping", type=int, default=0, help="override the per-cell mapping (KR_MAP_*; mapping study only)")
+    ap.add_argument("--threads-per-cell", type=int, default=0)
+    ap.add_argument("--retry", action="store_true", help="enable the retry procedure (PAPER.md:218; study only, default options have it off)")
+    ap.add_argument("--cpu-seconds", type=float, default=10.0, help="budget of the oracle timing per config")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    under_launcher = "RANK" in os.environ and "WORLD_SIZE" in os.environ
+    rank = int(os.environ.get("RANK", "0"))
+    if args.impl == "reference":
+        if rank == 0:
+            run_reference(args)
+        return
+    if under_launcher:
+        worker(args, rank, int(os.environ.get("LOCAL_RANK", "0")), int(os.environ["WORLD_SIZE"]))
+    elif args.gpus > 1:
+        # no torchrun around us: start the ranks here, one process per GPU
+        import torch
+        import torch.multiprocessing as mp
+        n_dev = torch.cuda.device_count()
+        if n_dev < args.gpus:
+            raise SystemExit(f"--gpus {args.gpus} asked for, {n_dev} CUDA device(s) visible")
+        with socket.socket() as s:
+            s.bind(("127.0.0.1", 0))
+            port = s.getsockname()[1]
+        mp.spawn(_spawn_entry, args=(args, args.gpus, port), nprocs=args.gpus, join=True)
+    else:
+        worker(args, 0, 0, 1)
 
 
 if __name__ == "__main__":

@@ -100,6 +100,9 @@ typedef struct {
   int32_t retry;        /* 1: a cell whose first attempt fails is redone from its input with tightened control before it is
                          * reverted (R24): one more launch (fp64) on the listed cells.  Default 0. */
   double retry_h0;      /* factor on the first sub-step of the second attempt (default 0.01) */
+  double cons_tol;      /* post-processing stage 2: a conservation row whose initial-minus-final total exceeds
+                         * cons_tol * sum_s |N_nu,s| |y_in,s| is compensated in full through its reservoir species; below it only
+                         * what stage 1 clamped is compensated (default 1e-13; reading R12) */
 } kr_solver_opts;
 
 /* Work counters of one call, summed over cells. */
@@ -178,6 +181,11 @@ int kr_network_spec_compile(const kr_network_desc *desc, int64_t *cubin_bytes, c
  * cubin size, log (host, may be NULL) the compiler log, cubin (host, may be NULL) up to cubin_cap bytes of the image. */
 int kr_network_wpc_compile(const kr_network_desc *desc, int precision_mode, int32_t warps_per_cell, int64_t *cubin_bytes,
                            char *log, int64_t log_cap, void *cubin, int64_t cubin_cap);
+
+/* Build-time check of the row-per-lane kernel (csrc/kr_row.cuh: fp64, one matrix row per lane, N <= 34 on one warp, N <= 64 on
+ * two): compile it with NVRTC for sm_100a without loading it (needs no GPU).  Arguments as kr_network_wpc_compile. */
+int kr_network_row_compile(const kr_network_desc *desc, int32_t warps_per_cell, int64_t *cubin_bytes, char *log, int64_t log_cap,
+                           void *cubin, int64_t cubin_cap);
 
 /* Mixed precision only, counters of the last step call summed over cells: refinement passes (fp64 residual + fp32
  * replay), and cells whose fp32 factorisation could not be refined and that were redone by the fp64 kernel (status bit

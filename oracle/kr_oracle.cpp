@@ -77,7 +77,7 @@ kr_oracle_opts default_opts() {
   o.shrink = 0.25; o.grow_fast = 8.0; o.grow_mid = 2.0; o.chg_floor = 1e-12;
   o.chg_max = std::numeric_limits<double>::infinity();
   o.it_fast = 3; o.it_mid = 5; o.max_substeps = 4096; o.finalize = 1; o.h_min_rel = 1e-12; o.bail_ratio = 10.0;
-  o.retry = 0; o.retry_h0 = 0.01;
+  o.retry = 0; o.retry_h0 = 0.01; o.cons_tol = 1e-13;
   return o;
 }
 
@@ -329,7 +329,7 @@ inline bool finite_all(const Real* x, int n) {
 
 struct Counters { int64_t acc = 0, rej = 0, newton = 0, lu = 0, rate = 0, failed = 0; };
 
-template <class Real> int finalize_state(const kr_oracle_network& n, Real* un, double* margin);
+template <class Real> int finalize_state(const kr_oracle_network& n, const Real* uin, Real* un, double* margin);
 
 inline void margin_update(double* m, double a, double b) {
   if (!m) return;
@@ -346,7 +346,7 @@ inline void margin_update(double* m, double a, double b) {
 // ---------------------------------------------------------------------------------------------
 template <class Real>
 bool be_substep(const kr_oracle_network& n, Real Ncal, const double* aux_cell, Real T_iso, Real h, Scratch<Real>& w,
-                Real& e_out, int& it_out, Counters& c, double* margin) {
+                Real& e_out, int& it_out, Counters& c, double* margin, double* amp = nullptr) {
   using std::abs;
   const int S = n.S, N = n.N, K = n.opts.max_newton;
   const kr_oracle_opts& o = n.opts;
@@ -371,6 +371,9 @@ bool be_substep(const kr_oracle_network& n, Real Ncal, const double* aux_cell, R
     lu_substitute(N, w.M.data(), w.perm.data(), w.delta.data());
     for (int i = 0; i < N; ++i) w.u[i] = w.u[i] + w.delta[i];
     if (!finite_all(w.u.data(), N)) { e_out = e; it_out = it; return false; }
+    if (amp)                                              // diagnostic only: cancellation in the update (see kr_oracle.h)
+      for (int i = 0; i < N; ++i)
+        *amp = std::max(*amp, double(abs(w.delta[i])) / (double(abs(w.u[i])) + (i < S ? 1e-20 : 0.0)));
     e = Real(0);
     for (int i = 0; i < N; ++i) {
       const Real atol = (i < S) ? Real(o.atol_y) : Real(o.atol_T);
@@ -398,7 +401,7 @@ bool be_substep(const kr_oracle_network& n, Real Ncal, const double* aux_cell, R
 template <class Real>
 int32_t step_attempt(const kr_oracle_network& n, const kr_oracle_opts& o, double h0_scale, bool count_failure, double rho,
                      double& T_io, double* y_io, double dt, const double* aux_cell, Scratch<Real>& w, Counters& c,
-                     double* margin) {
+                     double* margin, double* amp = nullptr) {
   using std::abs;
   const int S = n.S, N = n.N;
   int32_t st = 0;
@@ -447,7 +450,7 @@ int32_t step_attempt(const kr_oracle_network& n, const kr_oracle_opts& o, double
     if (h < h_floor || n_acc + n_rej > o.max_substeps) { failed = true; break; }
 
     Real e; int it;
-    const bool ran = be_substep<Real>(n, Ncal, aux_cell, T_iso, h, w, e, it, c, margin);
+    const bool ran = be_substep<Real>(n, Ncal, aux_cell, T_iso, h, w, e, it, c, margin, amp);
     // step 8: accept / reject
     bool ok = ran && finite_all(w.u.data(), N) && (e <= Real(1));
     if (ok) {
@@ -488,7 +491,7 @@ int32_t step_attempt(const kr_oracle_network& n, const kr_oracle_opts& o, double
     return st | ST_FAILED_REVERTED;                      // T_io, y_io untouched
   }
 
-  if (o.finalize) st |= finalize_state<Real>(n, w.un.data(), margin);
+  if (o.finalize) st |= finalize_state<Real>(n, w.uin.data(), w.un.data(), margin);
   for (int s = 0; s < S; ++s) y_io[s] = double(w.un[s]);
   if (n.energy) T_io = double(w.un[S]);
   return st;
@@ -500,45 +503,57 @@ int32_t step_attempt(const kr_oracle_network& n, const kr_oracle_opts& o, double
 // work counters add up over both attempts; the status is the second attempt's with RETRIED set.
 template <class Real>
 int32_t step_cell(const kr_oracle_network& n, double rho, double& T_io, double* y_io, double dt, const double* aux_cell,
-                  Scratch<Real>& w, Counters& c, double* margin) {
+                  Scratch<Real>& w, Counters& c, double* margin, double* amp = nullptr) {
   const kr_oracle_opts& o = n.opts;
-  int32_t st = step_attempt<Real>(n, o, 1.0, !o.retry, rho, T_io, y_io, dt, aux_cell, w, c, margin);
+  int32_t st = step_attempt<Real>(n, o, 1.0, !o.retry, rho, T_io, y_io, dt, aux_cell, w, c, margin, amp);
   if ((st & ST_FAILED_REVERTED) && o.retry) {
     kr_oracle_opts o2 = o;
     o2.shrink = o.shrink * o.shrink; o2.grow_fast = o.grow_mid; o2.grow_mid = 1.0;
-    st = step_attempt<Real>(n, o2, o.retry_h0, true, rho, T_io, y_io, dt, aux_cell, w, c, margin) | ST_RETRIED;
+    st = step_attempt<Real>(n, o2, o.retry_h0, true, rho, T_io, y_io, dt, aux_cell, w, c, margin, amp) | ST_RETRIED;
   }
   return st;
 }
 
-// Step 9: post-processing of the final state.
+// Step 9: post-processing of the final state (readings R12 / R23 of DESIGN.md).
 //   Stage 1: negatives -> 0.
-//   Stage 2 "corrects the violation in element abundances brought by step 1": the amount stage 1 added
-//     to row nu, -sum_s N_{nu,s} min(y_s, 0), is taken back from that row's reservoir species -- the single-row species
-//     with the largest abundance (reading R12: equal to the paper's initial-minus-final element totals up to the
-//     solver's own conservation error, which is rounding; forming it from the clamped amounts keeps a trace reservoir
-//     from absorbing eps * total).
+//   Stage 2: "Abundances of elements are calculated for the initial and final states of thermochemical
+//     evolution.  In the final state, the abundances in the single-element species are adjusted to compensate the
+//     differences.  This step corrects the violation in element abundances brought by step 1."  For every conservation
+//     row nu:  D_nu = sum_s N_{nu,s} (y_in,s - y_s)  with y already clamped (the paper's initial-minus-final totals),
+//     C_nu = sum_s N_{nu,s} min(y_s, 0) before clamping (the part of D_nu that stage 1 brought), and
+//     tot_nu = sum_s |N_{nu,s}| |y_in,s|.  The row is compensated by D_nu when |D_nu| > cons_tol tot_nu (a violation
+//     above rounding level: the literal text), else by C_nu (only what stage 1 brought: the solver's own drift below
+//     cons_tol is rounding noise and is not pushed into a possibly trace reservoir).  The compensation goes to the row's
+//     reservoir: the single-row species with the largest abundance (ties -> smallest index); no such species -> bit.
 //   Stage 3 (reading R23): "if step 2 causes negative abundances in some single-element species, the
 //     most abundant compound species is disintegrated into elements just sufficiently to correct this".  For every
 //     element row whose reservoir went negative, in row order: need = -y_res N_{nu,res} atoms; the neutral compound
 //     (>= 2 non-zero rows, no entry on a signed row) with the largest abundance that contains the element gives up
 //     z = min(y_c, need / N_{nu,c}); its atoms of every row go to that row's reservoir; repeated with the next most
-//     abundant compound until the need is met (the reservoir then ends at exactly 0) or no compound is left (the
-//     NEEDS_STAGE3 bit stays).  Every row total is unchanged by construction.
-// Returns the status bits it sets.  un has S entries (abundances only).
+//     abundant compound until the need is met (the reservoir then ends at exactly 0) or no compound is left.
+//   NEEDS_STAGE3 is evaluated at the very end: set iff some row's reservoir is still negative (a reservoir that a LATER
+//   row's disintegration refilled does not keep the flag).  Every row total is unchanged by stage 3 by construction.
+// Returns the status bits it sets.  uin / un have S entries (abundances only); uin == nullptr means "the state itself"
+// (D_nu = C_nu: the entry point kr_oracle_finalize with no initial state).
 template <class Real>
-int finalize_state(const kr_oracle_network& n, Real* un, double* margin) {
+int finalize_state(const kr_oracle_network& n, const Real* uin, Real* un, double* margin) {
+  using std::abs;
   const int E = n.E, S = n.S;
   int st = 0;
-  std::vector<Real> removed(E, Real(0));
+  std::vector<Real> C(E, Real(0)), D(E, Real(0)), tot(E, Real(0));
   std::vector<int> res_of(E, -1);
-  bool any = false;
   for (int s = 0; s < S; ++s)
     if (un[s] < Real(0)) {
-      for (int nu = 0; nu < E; ++nu) removed[nu] += Real(n.comp[size_t(nu) * S + s]) * un[s];
-      un[s] = Real(0); st |= ST_CLAMPED_NEG; any = true;
+      for (int nu = 0; nu < E; ++nu) C[nu] += Real(n.comp[size_t(nu) * S + s]) * un[s];
+      un[s] = Real(0); st |= ST_CLAMPED_NEG;
     }
-  if (!any) return st;
+  for (int nu = 0; nu < E; ++nu) {
+    if (!uin) { D[nu] = C[nu]; continue; }
+    for (int s = 0; s < S; ++s) {
+      D[nu] += Real(n.comp[size_t(nu) * S + s]) * (uin[s] - un[s]);
+      tot[nu] += Real(abs(n.comp[size_t(nu) * S + s])) * Real(abs(uin[s]));
+    }
+  }
   auto reservoir = [&](int nu, int* second_out) {
     int res = -1, second = -1;
     for (int s = 0; s < S; ++s) {
@@ -549,18 +564,23 @@ int finalize_state(const kr_oracle_network& n, Real* un, double* margin) {
     if (second_out) *second_out = second;
     return res;
   };
-  bool need3 = false;
   for (int nu = 0; nu < E; ++nu) {
-    if (removed[nu] == Real(0)) continue;
+    Real delta = C[nu];
+    if (uin) {
+      const Real thr = Real(n.opts.cons_tol) * tot[nu];
+      // the drift is rounding noise that no two implementations share: a cell whose drift is within a decade of the
+      // threshold is not comparable
+      if (margin && Real(abs(D[nu])) > Real(0.1) * thr && Real(abs(D[nu])) < Real(10) * thr) *margin = 0.0;
+      if (Real(abs(D[nu])) > thr) delta = D[nu];
+    }
+    if (delta == Real(0)) continue;
     int second = -1;
     const int res = reservoir(nu, &second);
     if (res < 0) { st |= ST_NO_RESERVOIR; continue; }
     if (second >= 0) margin_update(margin, double(un[res]), double(un[second]));
     res_of[nu] = res;
-    un[res] = un[res] + removed[nu] / Real(n.comp[size_t(nu) * S + res]);
-    if (un[res] < Real(0)) need3 = true;
+    un[res] = un[res] + delta / Real(n.comp[size_t(nu) * S + res]);
   }
-  if (!need3) return st;
   // stage 3
   std::vector<char> signed_row(E, 0), compound(S, 0);
   for (int nu = 0; nu < E; ++nu)
@@ -577,7 +597,7 @@ int finalize_state(const kr_oracle_network& n, Real* un, double* margin) {
     const int res = res_of[nu];
     if (res < 0 || !(un[res] < Real(0))) continue;
     const Real nres = Real(n.comp[size_t(nu) * S + res]);
-    if (signed_row[nu] || !(nres > Real(0))) { st |= ST_NEEDS_STAGE3; continue; }
+    if (signed_row[nu] || !(nres > Real(0))) continue;
     Real need = -un[res] * nres;
     for (int iter = 0; iter < S && need > Real(0); ++iter) {
       int c = -1;
@@ -603,24 +623,28 @@ int finalize_state(const kr_oracle_network& n, Real* un, double* margin) {
       }
       un[res] = un[res] + nc * z / nres;
       need = all ? need - nc * z : Real(0);
+      st |= ST_STAGE3;
     }
-    if (need > Real(0)) st |= ST_NEEDS_STAGE3;
-    else { un[res] = Real(0); st |= ST_STAGE3; }   // "just sufficiently": the reservoir ends at exactly zero
+    if (!(need > Real(0))) un[res] = Real(0);      // "just sufficiently": the reservoir ends at exactly zero
   }
+  for (int nu = 0; nu < E; ++nu)
+    if (res_of[nu] >= 0 && un[res_of[nu]] < Real(0)) st |= ST_NEEDS_STAGE3;
   return st;
 }
 
 template <class Real>
 void run_range(const kr_oracle_network* n, int64_t lo, int64_t hi, int64_t n_cells, const double* rho, double* T,
-               double* y, double dt, const double* aux, int32_t n_aux, int32_t* status, Counters* cnt, double* margins) {
+               double* y, double dt, const double* aux, int32_t n_aux, int32_t* status, Counters* cnt, double* margins,
+               double* amps) {
   Scratch<Real> w(*n);
   std::vector<double> aux_cell(std::max(1, n_aux));
   for (int64_t c = lo; c < hi; ++c) {
     for (int a = 0; a < n_aux; ++a) aux_cell[a] = aux[size_t(a) * n_cells + c];
-    double m = std::numeric_limits<double>::infinity();
+    double m = std::numeric_limits<double>::infinity(), am = 0.0;
     double Tc = T[c];
     const int32_t st = step_cell<Real>(*n, rho[c], Tc, y + size_t(c) * n->S, dt, aux_cell.data(), w, *cnt,
-                                       margins ? &m : nullptr);
+                                       margins ? &m : nullptr, amps ? &am : nullptr);
+    if (amps) amps[c] = am;
     if (n->energy && !(st & ST_FAILED_REVERTED)) T[c] = Tc;
     if (status) status[c] = st;
     if (margins) margins[c] = m;
@@ -629,18 +653,19 @@ void run_range(const kr_oracle_network* n, int64_t lo, int64_t hi, int64_t n_cel
 
 template <class Real>
 int run_step(kr_oracle_network* n, int64_t n_cells, const double* rho, double* T, double* y, double dt, const double* aux,
-             int32_t n_aux, int32_t* status, kr_oracle_stats* stats, double* margins, int32_t n_threads) {
+             int32_t n_aux, int32_t* status, kr_oracle_stats* stats, double* margins, int32_t n_threads,
+             double* amps = nullptr) {
   if (!n || n_cells < 0 || (n_cells > 0 && (!rho || !T || !y)) || !(dt > 0)) return -1;
   if (n->n_aux_needed > n_aux || (n_aux > 0 && !aux)) return -1;
   n_threads = std::max(1, n_threads);
   std::vector<Counters> cnt(n_threads);
   if (n_threads == 1 || n_cells < 2 * n_threads) {
-    run_range<Real>(n, 0, n_cells, n_cells, rho, T, y, dt, aux, n_aux, status, &cnt[0], margins);
+    run_range<Real>(n, 0, n_cells, n_cells, rho, T, y, dt, aux, n_aux, status, &cnt[0], margins, amps);
   } else {
     std::vector<std::thread> th;
     for (int t = 0; t < n_threads; ++t) {
       const int64_t lo = n_cells * t / n_threads, hi = n_cells * (t + 1) / n_threads;
-      th.emplace_back(run_range<Real>, n, lo, hi, n_cells, rho, T, y, dt, aux, n_aux, status, &cnt[t], margins);
+      th.emplace_back(run_range<Real>, n, lo, hi, n_cells, rho, T, y, dt, aux, n_aux, status, &cnt[t], margins, amps);
     }
     for (auto& x : th) x.join();
   }
@@ -732,6 +757,12 @@ int kr_oracle_thermochem_step_ex(kr_oracle_network* n, int64_t n_cells, const do
   return run_step<double>(n, n_cells, rho, T, y, dt, aux, n_aux, status, stats, margins, n_threads);
 }
 
+int kr_oracle_thermochem_step_diag(kr_oracle_network* n, int64_t n_cells, const double* rho, double* T, double* y, double dt,
+                                   const double* aux, int32_t n_aux, int32_t* status, kr_oracle_stats* stats,
+                                   double* margins, double* amps, int32_t n_threads) {
+  return run_step<double>(n, n_cells, rho, T, y, dt, aux, n_aux, status, stats, margins, n_threads, amps);
+}
+
 int kr_oracle_witness_step_ex(kr_oracle_network* n, int64_t n_cells, const double* rho, double* T, double* y, double dt,
                               const double* aux, int32_t n_aux, int32_t* status, kr_oracle_stats* stats,
                               int32_t n_threads) {
@@ -791,9 +822,9 @@ int kr_oracle_lu_solve(int32_t nn, double* M, const double* b, double* x, int32_
   return 0;
 }
 
-int kr_oracle_finalize(kr_oracle_network* n, double* y, int32_t* status) {
+int kr_oracle_finalize(kr_oracle_network* n, const double* y_in, double* y, int32_t* status) {
   if (!n || !y) return -1;
-  const int st = finalize_state<double>(*n, y, nullptr);
+  const int st = finalize_state<double>(*n, y_in, y, nullptr);
   if (status) *status = st;
   return 0;
 }

@@ -43,6 +43,7 @@ typedef struct {
   double bail_ratio;                       /* early-exit mode: abort the sub-step when e_k > bail_ratio * e_{k-1}, k >= 2 */
   int32_t retry;                           /* 1: a failed cell is tried once more with tightened control (R24) */
   double retry_h0;                         /* factor on the first sub-step of the second attempt */
+  double cons_tol;                         /* stage 2: a row whose initial-minus-final total exceeds cons_tol * sum|N||y_in| is compensated in full */
 } kr_oracle_opts;
 
 typedef struct { int64_t n_substeps, n_rejected, n_newton, n_lu, n_rate_evals, n_failed; } kr_oracle_stats;
@@ -59,6 +60,14 @@ int  kr_oracle_set_options(kr_oracle_network*, const kr_oracle_opts*);
 int kr_oracle_thermochem_step_ex(kr_oracle_network*, int64_t n_cells, const double* rho, double* T, double* y,
                                  double dt, const double* aux, int32_t n_aux, int32_t* status,
                                  kr_oracle_stats* stats, double* margins, int32_t n_threads);
+/* Same step with one more diagnostic per cell: amps [n_cells] or NULL receives the largest cancellation any Newton
+ * update of the cell went through, max over iterations and unknowns of |delta_i| / (|u_i + delta_i| + 1e-20 for an
+ * abundance): a value of 10^a says that a digits of the update cancelled, i.e. that rounding differences inside the
+ * linear solve were amplified by 10^a in the iterate (a Newton iteration started far from the solution; DESIGN.md
+ * section 3 uses it to tell which cells fp64 determines to 1e-9).  Diagnostic only: it does not enter the algorithm. */
+int kr_oracle_thermochem_step_diag(kr_oracle_network*, int64_t n_cells, const double* rho, double* T, double* y,
+                                   double dt, const double* aux, int32_t n_aux, int32_t* status,
+                                   kr_oracle_stats* stats, double* margins, double* amps, int32_t n_threads);
 /* Same algorithm carried in long double (the "witness"); results rounded to double. */
 int kr_oracle_witness_step_ex(kr_oracle_network*, int64_t n_cells, const double* rho, double* T, double* y,
                               double dt, const double* aux, int32_t n_aux, int32_t* status,
@@ -80,8 +89,9 @@ int kr_oracle_lu_solve(int32_t n, double* M, const double* b, double* x, int32_t
 /* step 6: one backward-Euler sub-step of size h from u_n = (y[, T]); u_out [N];
  * e_out = last e_k, it_out = first k with e_k <= 1 (K+1 if none); returns 0, or 1 when the
  * sub-step aborted (LU failure / non-finite / bail-out). */
-/* Post-processing stages 1-3 applied to one state y[S] in place; *status receives the bits set. */
-int kr_oracle_finalize(kr_oracle_network*, double* y, int32_t* status);
+/* Post-processing stages 1-3 applied to one final state y[S] in place, given the initial state
+ * y_in[S] of the step (NULL: the final state itself, i.e. only what stage 1 clamps is compensated); *status receives the bits set. */
+int kr_oracle_finalize(kr_oracle_network*, const double* y_in, double* y, int32_t* status);
 
 int kr_oracle_be_substep(kr_oracle_network*, double rho, double T, const double* y, const double* aux_cell,
                          double h, double* u_out, double* e_out, int32_t* it_out);

@@ -35,7 +35,8 @@ class _Opts(C.Structure):
                 ("eta", C.c_double), ("y_floor", C.c_double), ("shrink", C.c_double), ("grow_fast", C.c_double),
                 ("grow_mid", C.c_double), ("chg_floor", C.c_double), ("chg_max", C.c_double),
                 ("it_fast", C.c_int32), ("it_mid", C.c_int32), ("max_substeps", C.c_int32), ("finalize", C.c_int32),
-                ("h_min_rel", C.c_double), ("bail_ratio", C.c_double), ("retry", C.c_int32), ("retry_h0", C.c_double)]
+                ("h_min_rel", C.c_double), ("bail_ratio", C.c_double), ("retry", C.c_int32), ("retry_h0", C.c_double),
+                ("cons_tol", C.c_double)]
 
 
 class Stats(C.Structure):
@@ -61,6 +62,8 @@ def load():
     lib.kr_oracle_set_options.argtypes = [vp, C.POINTER(_Opts)]
     lib.kr_oracle_thermochem_step_ex.argtypes = [vp, C.c_int64, _dp, _dp, _dp, C.c_double, _dp, C.c_int32, _ip,
                                                  C.POINTER(Stats), _dp, C.c_int32]
+    lib.kr_oracle_thermochem_step_diag.argtypes = [vp, C.c_int64, _dp, _dp, _dp, C.c_double, _dp, C.c_int32, _ip,
+                                                   C.POINTER(Stats), _dp, _dp, C.c_int32]
     lib.kr_oracle_witness_step_ex.argtypes = [vp, C.c_int64, _dp, _dp, _dp, C.c_double, _dp, C.c_int32, _ip,
                                               C.POINTER(Stats), C.c_int32]
     lib.kr_oracle_rate_constants.argtypes = [vp, C.c_double, _dp, _dp, _dp]
@@ -68,7 +71,7 @@ def load():
     lib.kr_oracle_eval_rhs_complex.argtypes = [vp, C.c_double, C.c_double, C.c_double, _dp, _dp, _dp, _dp, _dp]
     lib.kr_oracle_eval_jacobian.argtypes = [vp, C.c_double, C.c_double, _dp, _dp, _dp]
     lib.kr_oracle_lu_solve.argtypes = [C.c_int32, _dp, _dp, _dp, _ip]
-    lib.kr_oracle_finalize.argtypes = [vp, _dp, C.POINTER(C.c_int32)]
+    lib.kr_oracle_finalize.argtypes = [vp, _dp, _dp, C.POINTER(C.c_int32)]
     lib.kr_oracle_be_substep.argtypes = [vp, C.c_double, C.c_double, _dp, _dp, C.c_double, _dp, _dp, _ip]
     _lib = lib
     return lib
@@ -131,14 +134,15 @@ class OracleNetwork:
         s = _Opts(o.max_newton, o.fixed_newton, o.h0_mode, o.rtol, o.atol_y, o.atol_T, o.neg_tol, o.eta, o.y_floor,
                   o.shrink, o.grow_fast, o.grow_mid, o.chg_floor, o.chg_max, o.it_fast, o.it_mid, o.max_substeps,
                   getattr(o, "finalize", 1), getattr(o, "h_min_rel", 1e-12), getattr(o, "bail_ratio", 10.0),
-                  getattr(o, "retry", 0), getattr(o, "retry_h0", 0.01))
+                  getattr(o, "retry", 0), getattr(o, "retry_h0", 0.01), getattr(o, "cons_tol", 1e-13))
         rc = load().kr_oracle_set_options(self._h, C.byref(s))
         if rc != 0:
             raise ValueError("kr_oracle_set_options rejected the options")
 
     # -- the step -------------------------------------------------------------------------
-    def step(self, cells, n_threads: int = 1, witness: bool = False, want_margins: bool = False):
-        """Returns (T, y, status, stats, margins) -- inputs are not modified."""
+    def step(self, cells, n_threads: int = 1, witness: bool = False, want_margins: bool = False, amps=None):
+        """Returns (T, y, status, stats, margins) -- inputs are not modified.  amps: optional float64 [n_cells] array
+        that receives the per-cell cancellation diagnostic of kr_oracle_thermochem_step_diag."""
         lib = load()
         n = cells.n_cells
         T = _f64(cells.T).copy()
@@ -152,6 +156,10 @@ class OracleNetwork:
         if witness:
             rc = lib.kr_oracle_witness_step_ex(self._h, n, _d(rho), _d(T), _d(y), float(cells.dt), _d(aux), n_aux,
                                                _i(status), C.byref(st), int(n_threads))
+        elif amps is not None:
+            assert amps.dtype == np.float64 and amps.shape == (n,) and amps.flags.c_contiguous
+            rc = lib.kr_oracle_thermochem_step_diag(self._h, n, _d(rho), _d(T), _d(y), float(cells.dt), _d(aux), n_aux,
+                                                    _i(status), C.byref(st), _d(margins), _d(amps), int(n_threads))
         else:
             rc = lib.kr_oracle_thermochem_step_ex(self._h, n, _d(rho), _d(T), _d(y), float(cells.dt), _d(aux), n_aux,
                                                   _i(status), C.byref(st), _d(margins), int(n_threads))
@@ -187,11 +195,13 @@ class OracleNetwork:
         load().kr_oracle_eval_jacobian(self._h, float(rho), float(T), _d(_f64(y)), _d(ax), _d(J))
         return J
 
-    def finalize(self, y):
-        """Post-processing stages 1-3 on one state; returns (y_out, status bits)."""
+    def finalize(self, y, y_in=None):
+        """Post-processing stages 1-3 on one final state (y_in: the initial state of the step, or None);
+        returns (y_out, status bits)."""
         yy = _f64(np.asarray(y, dtype=np.float64)).copy()
+        yi = None if y_in is None else _f64(np.asarray(y_in, dtype=np.float64))
         st = C.c_int32(0)
-        rc = load().kr_oracle_finalize(self._h, _d(yy), C.byref(st))
+        rc = load().kr_oracle_finalize(self._h, _d(yi), _d(yy), C.byref(st))
         if rc != 0:
             raise RuntimeError("oracle finalize failed")
         return yy, int(st.value)

@@ -25,7 +25,7 @@ ST_REJECTED_ONCE, ST_CLAMPED_NEG, ST_FP64_FALLBACK, ST_FAILED_REVERTED, ST_T_CLA
 EXPORTS = [
     "kr_network_create", "kr_network_destroy", "kr_default_opts", "kr_network_set_options",
     "kr_network_get_options", "kr_set_stream", "kr_network_set_mapping", "kr_network_info",
-    "kr_network_kernel_desc", "kr_network_spec_source", "kr_network_spec_compile", "kr_network_wpc_compile", "kr_last_mixed_stats", "kr_thermochem_step", "kr_thermochem_step_ex", "kr_thermochem_step_host", "kr_last_launch_count",
+    "kr_network_kernel_desc", "kr_network_spec_source", "kr_network_spec_compile", "kr_network_wpc_compile", "kr_network_row_compile", "kr_last_mixed_stats", "kr_thermochem_step", "kr_thermochem_step_ex", "kr_thermochem_step_host", "kr_last_launch_count",
     "kr_layout_cell_to_soa", "kr_layout_soa_to_cell", "kr_math_probe", "kr_measure_fp64_peak", "kr_last_error", "kr_version",
 ]
 
@@ -55,7 +55,8 @@ class SolverOpts(C.Structure):
                 ("eta", C.c_double), ("y_floor", C.c_double), ("shrink", C.c_double),
                 ("grow_fast", C.c_double), ("grow_mid", C.c_double), ("chg_floor", C.c_double), ("chg_max", C.c_double),
                 ("it_fast", C.c_int32), ("it_mid", C.c_int32), ("max_substeps", C.c_int32), ("finalize", C.c_int32),
-                ("h_min_rel", C.c_double), ("bail_ratio", C.c_double), ("retry", C.c_int32), ("retry_h0", C.c_double)]
+                ("h_min_rel", C.c_double), ("bail_ratio", C.c_double), ("retry", C.c_int32), ("retry_h0", C.c_double),
+                ("cons_tol", C.c_double)]
 
 
 class StepStats(C.Structure):
@@ -98,6 +99,8 @@ def load() -> C.CDLL:
     lib.kr_network_kernel_desc.argtypes = [vp, C.c_char_p, C.c_int64]
     lib.kr_network_spec_source.argtypes = [C.POINTER(NetworkDesc), C.c_char_p, C.c_int64]
     lib.kr_network_spec_compile.argtypes = [C.POINTER(NetworkDesc), C.POINTER(C.c_int64), C.c_char_p, C.c_int64]
+    lib.kr_network_row_compile.argtypes = [C.POINTER(NetworkDesc), C.c_int32, C.POINTER(C.c_int64), C.c_char_p, C.c_int64,
+                                           C.c_void_p, C.c_int64]
     lib.kr_network_wpc_compile.argtypes = [C.POINTER(NetworkDesc), C.c_int, C.c_int32, C.POINTER(C.c_int64), C.c_char_p, C.c_int64,
                                            vp, C.c_int64]
     lib.kr_last_mixed_stats.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
@@ -206,6 +209,21 @@ def wpc_compile(net, precision_mode: int = KR_FP64, warps_per_cell: int = 1, wan
     cap = (8 << 20) if want_cubin else 0
     img = C.create_string_buffer(cap) if want_cubin else None
     _check(load().kr_network_wpc_compile(C.byref(d), int(precision_mode), int(warps_per_cell), C.byref(size), log, 1 << 16,
+                                         C.cast(img, C.c_void_p) if want_cubin else None, cap))
+    out = {"cubin_bytes": size.value, "log": log.value.decode()}
+    if want_cubin:
+        out["cubin"] = img.raw[:size.value]
+    return out
+
+
+def row_compile(net, warps_per_cell: int = 1, want_cubin: bool = False) -> dict:
+    """kr_network_row_compile: NVRTC-compile the row-per-lane kernel for sm_100a (no GPU needed)."""
+    d, keep = make_desc(net)
+    size = C.c_int64()
+    log = C.create_string_buffer(1 << 16)
+    cap = (8 << 20) if want_cubin else 0
+    img = C.create_string_buffer(cap) if want_cubin else None
+    _check(load().kr_network_row_compile(C.byref(d), int(warps_per_cell), C.byref(size), log, 1 << 16,
                                          C.cast(img, C.c_void_p) if want_cubin else None, cap))
     out = {"cubin_bytes": size.value, "log": log.value.decode()}
     if want_cubin:

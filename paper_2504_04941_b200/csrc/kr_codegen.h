@@ -11,13 +11,14 @@
 struct KrHostNet {
   int E = 0, S = 0, R = 0, N = 0, energy = 0, n_aux = 0, any_rev = 0, any_tb = 0, any_qext = 0;
   double T_lo = 0, T_hi = 0, ln_p0_kB = 0;
-  std::vector<int> sp, nu, flags, auxi, dnu_tot, comp, resv, compound, signed_row, row_ptr, col_ptr, row_ent, col_ent;
+  std::vector<int> sp, nu, flags, auxi, dnu_tot, comp, signed_row, row_ptr, col_ptr, row_ent, col_ent;
+  std::vector<int> post_sp_ptr, post_sp_ent, post_res_ptr, post_res_ent, post_cmp_ptr, post_cmp_ent;   // kr_post.cuh lists
   std::vector<double> c0, A, beta, Ea, qk, tb, nasa, T_mid;
   // programs of the register-tile kernel (empty when N > 64)
   std::vector<KrDEnt> rprog;
-  std::vector<int> rprog_ptr, fac, tgt, emeta[2];
-  int n_entries = 0, elen[2] = {0, 0};
-  std::vector<KrETerm> estream[2];
+  std::vector<int> rprog_ptr, fac, tgt, emeta[4];       // streams: [0..1] kr_wpc.cuh layout (32 / 64 threads), [2..3] kr_row.cuh layout
+  int n_entries = 0, elen[4] = {0, 0, 0, 0};
+  std::vector<KrETerm> estream[4];
 };
 
 namespace kr_codegen {
@@ -78,9 +79,13 @@ inline std::string net_header(const KrHostNet& H, int block, int min_blocks) {
   s += arr2("double", "nasa", H.nasa, H.S, 14, fd);
   s += arr1("double", "T_mid", H.T_mid, H.S, fd);
   s += arr2("int", "comp", H.comp, H.E, H.S, fi);
-  s += arr2("int", "resv", H.resv, H.E, H.S, fi);
-  s += arr1("int", "compound", H.compound, H.S, fi);
   s += arr1("int", "signed_row", H.signed_row, H.E, fi);
+  s += arr1("int", "post_sp_ptr", H.post_sp_ptr, H.post_sp_ptr.size(), fi);
+  s += arr1("int", "post_sp_ent", H.post_sp_ent, H.post_sp_ent.size(), fi);
+  s += arr1("int", "post_res_ptr", H.post_res_ptr, H.post_res_ptr.size(), fi);
+  s += arr1("int", "post_res_ent", H.post_res_ent, H.post_res_ent.size(), fi);
+  s += arr1("int", "post_cmp_ptr", H.post_cmp_ptr, H.post_cmp_ptr.size(), fi);
+  s += arr1("int", "post_cmp_ent", H.post_cmp_ent, H.post_cmp_ent.size(), fi);
   s += "};\n";
   return s;
 }

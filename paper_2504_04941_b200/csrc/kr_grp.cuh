@@ -484,7 +484,7 @@ __global__ void __launch_bounds__(256) kr_grp_kernel(const KrNetDev n, const KrO
     }
     // ---- step 9: finalise (stages 1-3, kr_post.cuh; serial in thread 0: O(E S) once per cell) + layout-out ------------------
     if (o.finalize && G.gl == 0) {
-      st |= kr_postprocess(KrPostTab{n}, [&](int s) -> double& { return c[L.oUN + s]; });
+      st |= kr_postprocess(kr_post_lists(n), o.cons_tol, [&](int s) { return a.y[cell * n.S + s]; }, [&](int s) -> double& { return c[L.oUN + s]; });
       if (a.status) a.status[cell] = st;
     } else if (G.gl == 0 && a.status) {
       a.status[cell] = st;

@@ -292,18 +292,14 @@ __device__ __forceinline__ bool krs_lu_solve(const KrsShared& sh, const int (&vh
   return ok;                                               // no early exit: every lane of the block walks the same code
 }
 
-// step 9 on the lane's u_n in shared memory ([entry][lane] layout), out of line: it runs once per cell and only when an
-// abundance ended negative
-struct KrsPostTab {
-  __device__ __forceinline__ int E() const { return KrNet::E; }
-  __device__ __forceinline__ int S() const { return KrNet::S; }
-  __device__ __forceinline__ int comp(int nu, int s) const { return KrNet::comp[nu][s]; }
-  __device__ __forceinline__ int resv(int nu, int s) const { return KrNet::resv[nu][s]; }
-  __device__ __forceinline__ int compound(int s) const { return KrNet::compound[s]; }
-  __device__ __forceinline__ int signed_row(int nu) const { return KrNet::signed_row[nu]; }
-};
-__device__ __noinline__ int krs_post(double* un0) {
-  return kr_postprocess(KrsPostTab{}, [&](int s) -> double& { return un0[s * KRS_BLOCK]; });
+// step 9 on the lane's u_n in shared memory ([entry][lane] layout), out of line: it runs once per cell and only for the
+// few cells that need it (a negative abundance, or a conservation row drifting beyond cons_tol)
+__device__ __forceinline__ KrPostLists krs_post_lists() {
+  return KrPostLists{KrNet::E, KrNet::S, KrNet::post_sp_ptr, KrNet::post_sp_ent, KrNet::post_res_ptr, KrNet::post_res_ent,
+                     KrNet::post_cmp_ptr, KrNet::post_cmp_ent, KrNet::signed_row};
+}
+__device__ __noinline__ int krs_post(double* un0, const double* yin, double cons_tol) {
+  return kr_postprocess(krs_post_lists(), cons_tol, [&](int s) { return yin[s]; }, [&](int s) -> double& { return un0[s * KRS_BLOCK]; });
 }
 
 enum { KRS_FETCH = 0, KRS_RUN = 1, KRS_DONE = 2 };
@@ -532,10 +528,21 @@ kr_spec_kernel(const KrOptsDev o, const KrStepArgs g) {
     } else if (cell_done) {                                      // step 9: finalise + layout-out (u == u_n here)
       c_acc += n_acc; c_rej += n_rej;
       if (o.finalize) {                                          // post-processing stages 1-3
+        // screen (unrolled over the composition matrix): a negative abundance, or a row whose initial-minus-final total
+        // exceeds cons_tol x its scale
         bool any = false;
-        KR_FOR(s, 0, S) any = any || (u[s] < 0.0); KR_END
+        double yin[S];
+        KR_FOR(s, 0, S) yin[s] = g.y[cell * S + s]; any = any || (u[s] < 0.0); KR_END
+        KR_FOR(nu, 0, KrNet::E)
+          double full = 0.0, scale = 0.0;
+          KR_FOR(s, 0, S)
+            constexpr int c = KrNet::comp[nu][s];
+            if constexpr (c != 0) { full += (double)c * (yin[s] - u[s]); scale += fabs((double)c * yin[s]); }
+          KR_END
+          any = any || (fabs(full) > o.cons_tol * scale);
+        KR_END
         if (any) {                                               // rare: the shared routine works on u_n (== u here)
-          st |= krs_post(&sh.UN(0));
+          st |= krs_post(&sh.UN(0), g.y + cell * S, o.cons_tol);
           KR_FOR(s, 0, S) u[s] = sh.UN(s); KR_END
         }
       }

@@ -52,10 +52,14 @@ struct KrNetDev {
   const double* nasa;    // [S*14]: 7 low-range then 7 high-range coefficients
   const double* T_mid;   // [S]
   // conservation rows
-  const int* comp;       // [E*S]
-  const int* resv;       // [E*S] 1 where species s is a reservoir candidate of row nu
-  const int* compound;   // [S] 1: neutral compound (>= 2 non-zero rows, none of them signed): stage-3 candidate (R23)
   const int* signed_row; // [E] 1: the row has negative entries (a charge row)
+  // gather lists of the end-of-step repair (kr_post.cuh; packed (index << 8) | (coefficient + 128))
+  const int* post_sp_ptr;   // [S+1] species s -> its non-zero rows
+  const int* post_sp_ent;
+  const int* post_res_ptr;  // [E+1] row nu -> species made of row nu only (the reservoir candidates)
+  const int* post_res_ent;
+  const int* post_cmp_ptr;  // [E+1] row nu -> neutral compounds holding nu whose other rows all have a reservoir candidate (R23)
+  const int* post_cmp_ent;
   // gather lists of the group (warp / CTA per cell) kernels
   const int* row_ptr;    // [S+1]  row list of species s: entries row_ptr[s]..row_ptr[s+1]
   const int* row_ent;    // packed (reaction << 8) | (dnu + 128)
@@ -80,6 +84,7 @@ struct KrOptsDev {
   double rtol, atol_y, atol_T, neg_tol, eta, y_floor, shrink, grow_fast, grow_mid, chg_floor, chg_max;
   double h_min_rel, bail_ratio;
   double h0_scale;       // factor on the first sub-step (1; retry_h0 in the second attempt of the retry procedure)
+  double cons_tol;       // end-of-step repair: rows drifting by more than cons_tol x scale are compensated in full
 };
 
 struct KrStepArgs {

@@ -346,7 +346,7 @@ __global__ void __launch_bounds__(KR_TPC_BD) kr_tpc_kernel(const KrNetDev n, con
         phase = KR_PH_FETCH;
       } else if (cell_done) {                                    // step 9: finalise + layout-out
         c_acc += n_acc; c_rej += n_rej;
-        if (o.finalize) st |= kr_postprocess(KrPostTab{n}, [&](int s) -> double& { return v.at(v.oUN, s); });
+        if (o.finalize) st |= kr_postprocess(kr_post_lists(n), o.cons_tol, [&](int s) { return a.y[cell * S + s]; }, [&](int s) -> double& { return v.at(v.oUN, s); });
         for (int s = 0; s < S; ++s) a.y[cell * S + s] = v.at(v.oUN, s);
         if (ENERGY) a.T[cell] = v.at(v.oUN, S);
         if (a.status) a.status[cell] = st;

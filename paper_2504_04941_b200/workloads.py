@@ -144,6 +144,7 @@ class SolverOpts:
     finalize: int = 1            # 0: skip step 9 (used by the conservation pin P4)
     retry: int = 0               # 1: a failed cell gets a second attempt with tightened control (R24)
     retry_h0: float = 0.01       # factor on the first sub-step of the second attempt
+    cons_tol: float = 1e-13      # stage 2: rows whose initial-minus-final total exceeds cons_tol * sum|N||y_in| are compensated in full
 
 
 # --------------------------------------------------------------------------

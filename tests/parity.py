@@ -32,7 +32,8 @@ def rel_err(y, y_ref, floor=FLOOR):
 
 def oracle_reference(oracle_mod, net, cells, opts, n_threads=8):
     on = oracle_mod.OracleNetwork(net, opts)
-    T, y, st, stats, margins = on.step(cells, n_threads=n_threads, want_margins=True)
+    amps = np.zeros(cells.n_cells)
+    T, y, st, stats, margins = on.step(cells, n_threads=n_threads, want_margins=True, amps=amps)
     Tw, yw, stw, _, _ = on.step(cells, n_threads=n_threads, witness=True)
     alpha = rel_err(y, yw).max(axis=1)
     if net.energy_equation:
@@ -51,7 +52,56 @@ def oracle_reference(oracle_mod, net, cells, opts, n_threads=8):
         gamma = np.maximum(gamma, np.where(stp == st, g, 1.0))
         margins = np.minimum(margins, mp)
     comparable = (alpha < 1e-11) & (margins > 1e-6) & (gamma < 1e-10) & ((st & 8) == 0) & ((stw & 8) == 0)
-    return dict(T=T, y=y, status=st, stats=stats, margins=margins, alpha=alpha, gamma=gamma, comparable=comparable)
+    return dict(T=T, y=y, status=st, stats=stats, margins=margins, alpha=alpha, gamma=gamma, comparable=comparable,
+                T_witness=Tw, y_witness=yw, status_witness=stw, amps=amps)
+
+
+def witness_error(ref, T, y, energy):
+    """Per-cell relative distance of a result (T, y) from the long-double witness of the oracle."""
+    err = rel_err(y, ref["y_witness"]).max(axis=1)
+    if energy:
+        err = np.maximum(err, np.abs(T - ref["T_witness"]) / np.abs(ref["T_witness"]))
+    return err
+
+
+# Cells that are not compared element by element (not comparable, or comparable but on a different accept path) still
+# have to be VALID outcomes: as close to the long-double witness as the fp64 oracle itself is, up to a factor and the
+# truncation error a different sub-step sequence can cause (backward Euler, rtol-controlled Newton: DESIGN.md section 3).
+UNMATCHED_FACTOR = 10.0
+UNMATCHED_SLACK = 1e-6
+# ... and a cell that really took another accept / reject path differs from the witness by the truncation error of a
+# first-order scheme whose step sizes follow the Newton iteration count, not an error estimate: bounded in the
+# mass-weighted norm sum|dy| / sum|y| (measured: <= 7e-2 on every such cell of configs 0-4)
+FLIPPED_MASS_WEIGHTED = 0.2
+
+
+def mass_weighted(y, y_ref):
+    return np.abs(y - y_ref).sum(axis=1) / np.maximum(np.abs(y_ref).sum(axis=1), 1e-300)
+
+
+def check_unmatched(net, ref, T_gpu, y_gpu, st_gpu, unmatched, slack=UNMATCHED_SLACK, max_violations=0.0):
+    """err(GPU, witness) <= 10 max(err(oracle64, witness), oracle's sensitivity to 1e-13 input perturbations) + slack on every cell of `unmatched` that neither side reverted;
+    returns the measured worst ratio.  max_violations: fraction of the unmatched cells that may exceed the bound (cells on
+    which fp64 itself is far from the witness -- reported)."""
+    m = unmatched & ((st_gpu & 8) == 0) & ((ref["status"] & 8) == 0) & ((ref["status_witness"] & 8) == 0)
+    if not m.any():
+        return dict(n_unmatched=int(unmatched.sum()), n_checked=0, worst=0.0, n_violations=0)
+    e_gpu = witness_error(ref, T_gpu, y_gpu, net.energy_equation)[m]
+    # the oracle's own rounding-level variability: its distance from the witness and how far its result moves under
+    # 1e-13 relative perturbations of the inputs (a chaotic Newton iteration started far from the solution can land on
+    # another root of the backward-Euler equations; such a cell bounds nothing)
+    e_ref = np.maximum(ref["alpha"], ref["gamma"])[m]
+    assert np.isfinite(y_gpu[m]).all()
+    bad = e_gpu > UNMATCHED_FACTOR * e_ref + slack
+    # the cells beyond the tight bound took another path: truncation-level agreement in the mass-weighted norm
+    mw_gpu = mass_weighted(y_gpu, ref["y_witness"])[m]
+    mw_ref = mass_weighted(ref["y"], ref["y_witness"])[m]
+    loose_bad = mw_gpu > UNMATCHED_FACTOR * mw_ref + FLIPPED_MASS_WEIGHTED
+    out = dict(n_unmatched=int(unmatched.sum()), n_checked=int(m.sum()), n_beyond_tight=int(bad.sum()),
+               worst_mass_weighted=float(mw_gpu.max()), n_beyond_loose=int(loose_bad.sum()))
+    assert bad.sum() <= max_violations * m.sum() + 1e-9, f"too many unmatched cells beyond the witness bound: {out}"
+    assert not loose_bad.any(), f"unmatched cells that are not valid outcomes at truncation level: {out}"
+    return out
 
 
 def element_drift(net, y_in, y_out):
@@ -62,19 +112,21 @@ def element_drift(net, y_in, y_out):
     return num / np.maximum(den, 1e-300)
 
 
-def compare(net, ref, T_gpu, y_gpu, st_gpu, tol=TOL, allow_path_flips=0.0):
+def compare(net, ref, T_gpu, y_gpu, st_gpu, tol=TOL, allow_path_flips=0.0, unmatched_slack=UNMATCHED_SLACK, unmatched_violations=0.05):
     """Returns a dict of measured quantities; raises AssertionError when a comparable cell is off.
 
     allow_path_flips: early-exit runs only -- fraction of comparable cells that may still have taken a
     different accept / early-exit path (several results are valid there; they are counted, reported, and
     must be finite and non-negative).  Fixed-K parity (the north_star bar) always uses 0."""
     m = ref["comparable"].copy()
+    unmatched = ~m
     if allow_path_flips > 0.0:
         rel0 = rel_err(y_gpu, ref["y"]).max(axis=1)
         flips = m & (rel0 > tol)
         assert flips.sum() <= allow_path_flips * max(int(m.sum()), 1), f"{int(flips.sum())} path flips of {int(m.sum())}"
         assert np.isfinite(y_gpu[flips]).all() and (y_gpu[flips] >= 0).all()
         m &= ~flips
+        unmatched = unmatched | flips
     rel = rel_err(y_gpu, ref["y"]).max(axis=1)
     relT = np.abs(T_gpu - ref["T"]) / np.abs(ref["T"])
     out = dict(n=int(m.size), n_comparable=int(m.sum()), max_rel_y=float(rel[m].max()) if m.any() else 0.0,
@@ -85,4 +137,6 @@ def compare(net, ref, T_gpu, y_gpu, st_gpu, tol=TOL, allow_path_flips=0.0):
     assert out["max_rel_y"] <= tol, f"abundance parity {out['max_rel_y']:.3e} > {tol} on comparable cells: {out}"
     assert out["max_rel_T"] <= tol, f"temperature parity {out['max_rel_T']:.3e} > {tol}: {out}"
     assert out["status_equal"] == 1.0, f"status bits differ on comparable cells: {out}"
+    out["unmatched"] = check_unmatched(net, ref, T_gpu, y_gpu, st_gpu, unmatched, slack=unmatched_slack,
+                                       max_violations=unmatched_violations)
     return out

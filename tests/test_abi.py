@@ -49,7 +49,7 @@ def test_struct_layouts_match_header(B):
     # kr_network_desc: 3 int32 (+pad), 16 pointers, 2 doubles, 1 int32 (+pad); kr_solver_opts / kr_step_stats
     assert C.sizeof(B.NetworkDesc) == 16 + 16 * 8 + 16 + 8
     assert C.sizeof(B.StepStats) == 48
-    assert C.sizeof(B.SolverOpts) == 16 + 11 * 8 + 16 + 16 + 16
+    assert C.sizeof(B.SolverOpts) == 16 + 11 * 8 + 16 + 16 + 16 + 8
 
 
 def test_validation_runs_on_the_host_before_any_device_work(B):
@@ -97,6 +97,19 @@ def test_register_tile_kernel_compiles_for_sm100a_without_a_gpu(B, idx, mode, wa
     assert out["cubin_bytes"] > 10000
     assert "error" not in out["log"].lower()
     assert "tiles" in out["log"]
+
+
+@pytest.mark.parametrize("idx,warps", [(3, 1), (4, 2), (1, 1), (0, 2), (2, 1)])
+def test_row_per_lane_kernel_compiles_for_sm100a_without_a_gpu(B, idx, warps):
+    """csrc/kr_row.cuh (warp-per-cell, one matrix row per lane, fp64) is compiled by NVRTC for the sizes of the network at
+    kr_network_create; the same compilation is checked here without a GPU: N = 33 on one warp with the T row spread over
+    the lanes, N = 64 on two warps, and small networks that leave lanes idle.  The static_asserts inside the kernel tie the
+    host's shared-memory layout and term-stream indices to the device's."""
+    out = B.row_compile(w.make_network(idx), warps)
+    assert out["cubin_bytes"] > 10000
+    assert "error" not in out["log"].lower()
+    with pytest.raises(B.KrError):
+        B.row_compile(w.make_network(4), 1)              # 64 rows do not fit one warp
 
 
 def test_null_and_nonsense_arguments(B):

@@ -11,9 +11,10 @@ from tests import parity as P
 pytestmark = pytest.mark.gpu
 
 # sizes: several thread blocks + a ragged tail; small enough for the oracle (+ witness) to finish in seconds
-SIZES = {0: 4096, 1: 1531, 2: 5003, 3: 203, 4: 70}
-# largest fraction of cells the protocol may exclude (fp64 itself does not resolve them; P10 in the oracle pins)
-MAX_EXCLUDED = {0: 0.08, 1: 0.01, 2: 0.01, 3: 0.03, 4: 0.45}
+SIZES = {0: 4096, 1: 1531, 2: 5003, 3: 1021, 4: 317}
+# largest fraction of cells the protocol may exclude (fp64 itself does not resolve them; P10 in the oracle pins);
+# measured fractions are listed in DESIGN.md section 3
+MAX_EXCLUDED = {0: 0.08, 1: 0.01, 2: 0.01, 3: 0.03, 4: 0.25}
 # config 0 takes h = dt first (h0_mode 0): Newton starts far from the solution and, for a few cells per thousand, amplifies
 # rounding differences by many decades before any decision -- those cells pass the oracle-side screens by chance only.
 # They are bounded here (<= 0.1 % in fixed-K mode) and must still be finite, non-negative and conserving.
@@ -48,13 +49,29 @@ def run_gpu(B, net, cells, opts, mode=0, mapping=None, tpc=0, host=False):
     return T.cpu().numpy(), y.cpu().numpy(), st.cpu().numpy()[:n], stats, gn
 
 
+FULL_SAMPLE = 16384          # every cell, else a seeded subset of >= 16 384
+_full_ref_cache = {}
+
+
+def full_size_reference(oracle_mod, idx, net, cells, opts):
+    """Seeded sample of FULL_SAMPLE cells of the full-size batch + its oracle reference (double, witness, margins,
+    perturbation screen), computed once per config and shared by the fp64 and mixed full-size tests."""
+    import os
+    if idx not in _full_ref_cache:
+        pick = np.sort(np.random.default_rng(99 + idx).choice(cells.n_cells, size=FULL_SAMPLE, replace=False))
+        _full_ref_cache[idx] = (pick, P.oracle_reference(oracle_mod, net, cells.take(pick), opts, n_threads=os.cpu_count() or 8))
+    return _full_ref_cache[idx]
+
+
 @pytest.mark.parametrize("fixed", [1, 0])
 @pytest.mark.parametrize("idx", [0, 1, 2, 3, 4])
 def test_parity_fp64(B, oracle_mod, idx, fixed):
     net, cells, opts = w.make_config(idx, SIZES[idx], fixed_newton=fixed)
     ref = P.oracle_reference(oracle_mod, net, cells, opts)
     T, y, st, stats, gn = run_gpu(B, net, cells, opts)
-    out = P.compare(net, ref, T, y, st, allow_path_flips=FIXED_K_FLIPS[idx] if fixed else 0.003)
+    out = P.compare(net, ref, T, y, st, allow_path_flips=FIXED_K_FLIPS[idx] if fixed else 0.003,
+                    unmatched_violations=0.25 if idx == 0 else 0.05)
+    print(f"parity fp64 config {idx} fixed={fixed}: {out}")
     assert 1.0 - out["n_comparable"] / out["n"] <= MAX_EXCLUDED[idx], out
     ok = (st & 8) == 0
     assert P.element_drift(net, cells.y[ok], y[ok]).max() <= 1e-12
@@ -87,7 +104,7 @@ def test_parity_mixed_precision(B, oracle_mod, idx, fixed):
     assert stats["n_failed"] <= ref["stats"]["n_failed"] + max(1, n // 100)
     ok = (st & 8) == 0
     assert np.isfinite(y).all()
-    assert P.element_drift(net, cells.y[ok], y[ok]).max() <= 1e-9
+    assert P.element_drift(net, cells.y[ok], y[ok]).max() <= 1e-12
     assert n_ref > 0 and stats["n_newton"] > 0
     # the fp64 work counters stay close to the oracle's: mixed precision must not buy speed with extra iterations
     assert stats["n_newton"] <= 1.6 * ref["stats"]["n_newton"] + 50
@@ -108,13 +125,15 @@ def test_register_tile_kernel_on_other_sizes(B, oracle_mod, S, energy, n_rev, mo
     T, y, st, stats, gn = run_gpu(B, net, cells, opts, mode=mode)
     desc = gn.kernel_desc()
     N = S + energy
-    assert ("register-tile" in desc) == (N <= 64), desc
+    assert (("row-per-lane" in desc) or ("register-tile" in desc)) == (N <= 64), desc
+    if mode == 0 and N <= 64:
+        assert "row-per-lane" in desc, desc
     out = P.compare(net, ref, T, y, st & ~B.ST_FP64_FALLBACK, tol=MIXED_TOL if mode else P.TOL,
                     allow_path_flips=0.03 if mode else 0.0)
     print(f"S={S} energy={energy} mode={mode}: {desc[:90]} {out}")
     assert out["n_comparable"] >= 0.6 * out["n"], out      # random thermochemistry: more cells fp64 itself does not resolve
     ok = (st & 8) == 0
-    assert P.element_drift(net, cells.y[ok], y[ok]).max() <= (1e-9 if mode else 1e-12)
+    assert P.element_drift(net, cells.y[ok], y[ok]).max() <= 1e-12
 
 
 @pytest.mark.parametrize("idx,n,mode", [(1, 3000, 0), (2, 5000, 0), (3, 2500, 0), (3, 2500, 1), (4, 400, 0), (4, 400, 1)])
@@ -208,9 +227,8 @@ def test_full_size_sampled_mixed(B, oracle_mod, idx):
     assert ok.mean() > 0.999 and np.isfinite(y).all() and (y >= 0).all()
     assert ms["n_fp64_cells"] == int(((st & B.ST_FP64_FALLBACK) != 0).sum())
     drift = P.element_drift(net, cells.y[ok], y[ok]).max(axis=1)
-    assert (drift > 1e-12).mean() <= 1e-4 and drift.max() <= 1e-9, float(drift.max())
-    pick = np.sort(np.random.default_rng(199 + idx).choice(n, size={3: 160, 4: 48}[idx], replace=False))
-    ref = P.oracle_reference(oracle_mod, net, cells.take(pick), opts)
+    assert drift.max() <= 1e-12, float(drift.max())          # north_star's bar, on every non-reverted cell
+    pick, ref = full_size_reference(oracle_mod, idx, net, cells, opts)
     out = P.compare(net, ref, T[pick], y[pick], st[pick] & ~B.ST_FP64_FALLBACK, tol=MIXED_TOL, allow_path_flips=MIXED_FLIPS[idx])
     print(f"full-size mixed config {idx}: {out} mixed={ms}")
 
@@ -219,7 +237,7 @@ def test_mixed_precision_needs_a_supported_size(B):
     import torch
     net = w.make_network(4)
     gn = B.Network(net)
-    assert "register-tile fp64" in gn.kernel_desc(), gn.kernel_desc()
+    assert "row-per-lane fp64" in gn.kernel_desc(), gn.kernel_desc()
 
 
 @pytest.mark.parametrize("idx,mapping,tpc", [(0, 4, 1), (1, 4, 1), (2, 4, 1), (1, 2, 32), (1, 3, 64), (2, 2, 32), (3, 3, 64),
@@ -448,6 +466,60 @@ def test_stream_argument_is_honoured(B, oracle_mod):
     np.testing.assert_array_equal(y1, yq)
 
 
+SUBSTEP_N = {0: 4096, 1: 4096, 2: 8192, 3: 1024, 4: 384}
+
+
+@pytest.mark.parametrize("q", [0.1, 0.5, 0.9])
+@pytest.mark.parametrize("idx,mapping,tpc", [(0, None, 0), (1, None, 0), (2, None, 0), (3, None, 0), (4, None, 0),      # default kernels
+                                             (1, 4, 1), (2, 4, 1), (3, 5, 32), (4, 5, 64), (3, 3, 64), (1, 2, 32)])      # every other family
+def test_single_substep_all_cells(B, oracle_mod, idx, mapping, tpc, q):
+    """ONE backward-Euler sub-step of K = 3 Newton iterations on EVERY cell, no controller decision: h = dt is taken as
+    it is (h0_mode 0), the sub-step is accepted whatever comes out (rtol, neg_tol huge), nothing is post-processed.  The
+    raw Newton iterate u^3 (negative values and all) must equal the oracle's on every cell: within 1e-9, or -- where the
+    long-double witness shows that fp64 does not resolve the linear systems that well -- within 50 x the oracle's own
+    distance from the witness.  h is the q-quantile of the cells' rate-based first sub-steps, so the batch spans
+    h k << 1 to h k >> 1.  Only cells whose T iterate leaves [T_lo, T_hi] (a rejection, hence a controller decision) or
+    whose iterates overflow are left out, and they are counted."""
+    import os
+    n = SUBSTEP_N[idx]
+    net, cells, opts = w.make_config(idx, n, fixed_newton=1)
+    on0 = oracle_mod.OracleNetwork(net, opts)
+    h0 = []
+    for c in range(0, n, max(1, n // 256)):
+        f = on0.rhs(cells.rho[c], float(np.clip(cells.T[c], net.T_lo, net.T_hi)), cells.y[c], None if cells.aux is None else cells.aux[:, c])
+        h0.append(opts.eta / max(np.max(np.abs(f[:net.n_species]) / (np.abs(cells.y[c]) + opts.y_floor)), 1e-300))
+    cells.dt = float(min(np.quantile(h0, q), cells.dt))
+    opts.h0_mode = 0; opts.max_newton = 3; opts.rtol = 1e30; opts.neg_tol = 1e30; opts.finalize = 0
+    on = oracle_mod.OracleNetwork(net, opts)
+    nt = os.cpu_count() or 8
+    amps = np.zeros(n)
+    To, yo, sto, statso, _ = on.step(cells, n_threads=nt, amps=amps)
+    Tw, yw, stw, _, _ = on.step(cells, n_threads=nt, witness=True)
+    # the oracle's step IS one be_substep on the cells it accepted at once (checked on a few cells through the piece itself)
+    clean = (sto & (1 | 8)) == 0
+    for c in np.nonzero(clean)[0][:8]:
+        u, e, it, rc = on.be_substep(cells.rho[c], float(np.clip(cells.T[c], net.T_lo, net.T_hi)), cells.y[c], cells.dt,
+                                     None if cells.aux is None else cells.aux[:, c])
+        assert rc == 0 and np.array_equal(u[:net.n_species], yo[c])
+    T, y, st, stats, gn = run_gpu(B, net, cells, opts, mapping=mapping, tpc=tpc)
+    use = clean & ((stw & (1 | 8)) == 0)
+    assert use.mean() >= 0.9, f"only {use.mean():.3f} of the cells took the single sub-step"
+    alpha = P.rel_err(yo, yw).max(axis=1)
+    err = P.rel_err(y, yo).max(axis=1)
+    if net.energy_equation:
+        alpha = np.maximum(alpha, np.abs(To - Tw) / np.abs(Tw))
+        err = np.maximum(err, np.abs(T - To) / np.abs(To))
+    # where an update cancelled a digits (amps = 10^a: Newton far from the solution), rounding inside the linear solve is
+    # amplified by 10^a in the iterate: such a cell cannot be asked for more than ~1e-13 x 10^a
+    tol = np.maximum(np.maximum(P.TOL, 50.0 * alpha), 1e-13 * amps)
+    bad = use & ~(err <= tol)
+    print(f"single sub-step config {idx} mapping {mapping} q={q}: h={cells.dt:.3e} cells used {int(use.sum())}/{n}, "
+          f"judged at 1e-9: {int((use & (tol <= P.TOL)).sum())}, max err {err[use].max():.2e}, max err/tol {np.max(err[use] / tol[use]):.2e}")
+    assert not bad.any(), f"{int(bad.sum())} cells off: worst err/tol {np.max(err[use] / tol[use]):.3e}"
+    assert ((st[use] & ~P.SIGN_BITS) == (sto[use] & ~P.SIGN_BITS)).all()
+    assert (use & (tol <= P.TOL)).sum() >= 0.5 * n        # most cells are judged at the north_star tolerance itself
+
+
 @pytest.mark.parametrize("idx", [1, 2, 3, 4])
 def test_full_size_sampled(B, oracle_mod, idx):
     """BASELINE sizes in the launch configuration bench.py times; the oracle recomputes a seeded sample of
@@ -461,13 +533,10 @@ def test_full_size_sampled(B, oracle_mod, idx):
     assert ok.mean() > 0.999
     assert np.isfinite(y).all() and (y >= 0).all()
     drift = P.element_drift(net, cells.y[ok], y[ok]).max(axis=1)
-    # 1e-12 (north_star).  Each Newton update conserves to rounding (~1e-16 relative), so the drift grows with the number
-    # of updates; config 4's stiffest cells take > 10^4 of them (up to 4096 sub-steps x 8 iterations) and 2 of 131 072
-    # were measured at 1.2e-12 (the table-driven LU kernel: 0.83e-12 on the same cells) -- those few are bounded at 1e-11.
-    assert (drift > 1e-12).mean() <= (1e-4 if idx == 4 else 0.0), float(drift.max())
-    assert drift.max() <= 1e-11
-    pick = np.sort(np.random.default_rng(99 + idx).choice(n, size={1: 1024, 2: 4096, 3: 160, 4: 48}[idx], replace=False))
-    sub = cells.take(pick)
-    ref = P.oracle_reference(oracle_mod, net, sub, opts)
+    # 1e-12 (north_star) on EVERY non-reverted cell: rows that drift beyond cons_tol = 1e-13 are restored from the
+    # initial totals by post-processing stage 2 (reading R12)
+    assert drift.max() <= 1e-12, float(drift.max())
+    pick, ref = full_size_reference(oracle_mod, idx, net, cells, opts)
     out = P.compare(net, ref, T[pick], y[pick], st[pick], allow_path_flips=0.003)
-    assert 1.0 - out["n_comparable"] / out["n"] <= MAX_EXCLUDED[idx] + 0.05, out
+    print(f"full-size config {idx}: {out}")
+    assert 1.0 - out["n_comparable"] / out["n"] <= MAX_EXCLUDED[idx], out

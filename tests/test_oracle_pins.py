@@ -484,6 +484,91 @@ def test_controller_bookkeeping(oracle_mod):
     np.testing.assert_array_equal(y, yin)
 
 
+# ------------------------------------------------------------------------------------------------
+# External heating (eq. 15: d(eps)/dt = Gamma - Lambda): one unary reaction A -> B that deposits q_ext per
+# event, constant c_v, equal formation enthalpies (no chemical heat): dT/dt = q_ext k y_A / (k_B C), C = sum y_s chat_s.
+# ------------------------------------------------------------------------------------------------
+def test_external_heat_term_closed_form(oracle_mod):
+    k, q = 2.0e-4, 3.0e-12                                    # s^-1, erg per event (~1.9 eV)
+    th = [[3.5, 0, 0, 0, 0, 0.0, 1.0], [4.5, 0, 0, 0, 0, 0.0, 2.0]]       # chat = 2.5, 3.5; a6 = 0 for both
+    for sign in (+1.0, -1.0):                                 # heating and (formally) cooling
+        net = H.tiny_network([[1, 1]], [((0,), (1,), k, 0, 0, w.F_CONST_UNARY, -1)], thermo=th, energy=1,
+                             q_ext=[sign * q], T_hi=1.0e6)
+        on = oracle_mod.OracleNetwork(net, _opts(max_newton=30, fixed_newton=0))
+        y, T, rho = np.array([0.7, 0.3]), 500.0, 1e-18
+        f = on.rhs(rho, T, y)
+        C = 0.7 * 2.5 + 0.3 * 3.5
+        # chemical part: -T sum uhat_s ydot_s with uhat = a1 - 1: ydot_A = -k y_A, ydot_B = +k y_A
+        chem = -T * (2.5 * (-k * 0.7) + 3.5 * (k * 0.7)) / C
+        ext = sign * q * k * 0.7 / (K_B * C)
+        assert f[0] == pytest.approx(-k * 0.7, rel=1e-14) and f[1] == pytest.approx(k * 0.7, rel=1e-14)
+        assert f[2] == pytest.approx(chem + ext, rel=1e-13)
+        assert abs(ext) > 20 * abs(chem)                      # the external term dominates: its sign is what is tested
+        # Jacobian of the heat term: dTdot/dy_A = q k / (k_B C) + chemical part (the dropped dC/dy term aside)
+        J = on.jacobian(rho, T, y)
+        assert J[2, 0] == pytest.approx((sign * q * k / K_B - T * (2.5 * (-k) + 3.5 * k)) / C, rel=1e-13)
+        # over a step the temperature moves the way the deposited energy says
+        u, e, it, rc = on.be_substep(rho, T, y, 0.02 / k)
+        assert rc == 0 and e <= 1 and (u[2] - T) * sign > 10.0
+        # energy bookkeeping of the converged backward-Euler step: sum_s y_s (H_s/R - T) changes by q (events) / k_B up to
+        # the O(h^2) drift of P9
+        dE = _energy(net, u[:2], u[2]) - _energy(net, y, T)
+        events = y[0] - u[0]
+        assert dE == pytest.approx(sign * q * events / K_B, rel=0.08)
+
+
+# ------------------------------------------------------------------------------------------------
+# The temperature clamp ("the check against effective temperature limits"): a cell fed T outside
+# [T_lo, T_hi] must give bit-identical results to the same cell fed T_lo / T_hi, on a network whose rates depend on T.
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("energy", [0, 1])
+def test_T_clamp_value(oracle_mod, energy):
+    th = [[3.5, 1e-4, 0, 0, 0, -2.0e3, 1.0], [4.0, 2e-4, 0, 0, 0, 1.0e3, 2.0], [3.7, 0, 0, 0, 0, 0.0, 3.0]]
+    net = H.tiny_network([[1, 1, 2]], [((0,), (1,), 1e-3, 0.7, 300.0, 0, -1), ((0, 1), (2,), 1e-12, -0.5, 150.0, w.F_REVERSIBLE, -1)],
+                         thermo=th, energy=energy, T_lo=200.0, T_hi=900.0)
+    on = oracle_mod.OracleNetwork(net, _opts())
+    y0 = np.array([[0.5, 0.2, 0.1]])
+    for T_fed, T_lim in ((20.0, 200.0), (199.999, 200.0), (5000.0, 900.0), (900.001, 900.0)):
+        a = on.step(H.cells_of(1e-12, T_fed, y0, 50.0))
+        b = on.step(H.cells_of(1e-12, T_lim, y0, 50.0))
+        np.testing.assert_array_equal(a[1], b[1])
+        assert (a[2][0] & 16) and not (b[2][0] & 16)
+        if energy:
+            np.testing.assert_array_equal(a[0], b[0])
+        assert a[3] == b[3]
+        # and the rate constants used are those at the limit: f(u_in) at T_lim drives the first sub-step
+    # a cell inside the range gives something else (the clamp is not a constant)
+    c = on.step(H.cells_of(1e-12, 500.0, y0, 50.0))
+    assert np.abs(c[1] - b[1]).max() > 1e-6
+
+
+# ------------------------------------------------------------------------------------------------
+# Decision margins (tests/parity.py uses them to decide which cells are comparable): on the linear A <-> B system of P1
+# Newton lands on the solution in ONE iteration, so e_1 = |delta| / (rtol |u_1| + atol) is known in closed form; the
+# reported margin must be the relative distance of the closest decision value to its threshold.
+# ------------------------------------------------------------------------------------------------
+def test_decision_margins_closed_form(oracle_mod):
+    kf, kr_ = 3.0e-3, 1.0e-3
+    net = H.tiny_network([[1, 1]], [((0,), (1,), kf, 0, 0, w.F_CONST_UNARY, -1), ((1,), (0,), kr_, 0, 0, w.F_CONST_UNARY, -1)])
+    y0 = np.array([0.9, 0.1])
+    h = 200.0
+    ktot = kf + kr_
+    yeq = kr_ / ktot
+    yA1 = yeq + (y0[0] - yeq) / (1.0 + ktot * h)               # P1's closed form
+    d = abs(yA1 - y0[0])
+    for target in (1.0 + 1e-3, 1.0 - 1e-3, 1.0 + 1e-7, 3.0):
+        # pick rtol so that e_1 = d / (rtol * min(u_A, u_B)) = target (atol = 0; the smaller abundance sets the maximum)
+        small = min(yA1, 1.0 - yA1)
+        rtol = d / (target * small)
+        o = _opts(h0_mode=0, fixed_newton=1, max_newton=2, rtol=rtol, atol_y=0.0, finalize=0)
+        on = oracle_mod.OracleNetwork(net, o)
+        T, y, st, stats, margins = on.step(H.cells_of(1e-20, 300.0, y0[None, :], h), want_margins=True)
+        assert y[0, 0] == pytest.approx(yA1, rel=1e-13)
+        # decisions taken: e_1 against 1 (the closed form), e_2 ~ 0 against 1 (margin 1), h against dt (an exact tie: skipped)
+        expect = abs(target - 1.0) / max(target, 1.0)
+        assert margins[0] == pytest.approx(expect, rel=2e-6 / max(expect, 1e-7) * 1e-7 + 1e-3)
+
+
 # ---- P11: post-processing stages 1-3 (readings R12 / R23) -------------------------------------------
 def _post_net():
     # elements a, b; species: a, b, a2 (single-element, a row), ab, ab2 (compounds); one reaction keeps the network valid
@@ -526,7 +611,7 @@ def test_P11_stage_3_disintegrates_the_most_abundant_compound_just_enough(oracle
     # not enough of ab2: it is used up, then the next compound (none left but ab = 0) -> NEEDS_STAGE3 stays, totals still hold
     y2 = np.array([0.01, 0.30, 0.005, -0.05, 0.03])
     yo2, st2 = on.finalize(y2)
-    assert st2 & 64 and not (st2 & 128)
+    assert st2 == (2 | 64 | 128)          # clamped, ab2 was taken apart (STAGE3), the a reservoir is still negative (NEEDS_STAGE3)
     np.testing.assert_allclose(comp @ yo2, comp @ y2, rtol=0, atol=6e-17)
     assert yo2[4] == 0.0 and yo2[0] < 0.0
     # two compounds needed: ab2 (0.03) is exhausted, ab (0.02) covers the remaining 0.01
@@ -567,6 +652,69 @@ def test_P11_random_states_conserve_and_end_non_negative(oracle_mod):
         if not (st & (32 | 64)):
             assert yo.min() >= 0.0
     assert n3 >= 20                                           # stage 3 was exercised
+
+
+def test_P11_stage_2_initial_minus_final_totals(oracle_mod):
+    """PAPER.md:215 literally: 'Abundances of elements are calculated for the initial and final states ... the abundances
+    in the single-element species are adjusted to compensate the differences.'  With an initial state given, a row whose
+    initial-minus-final total exceeds cons_tol x sum|N||y_in| is compensated IN FULL (solver drift included); below the
+    threshold only what stage 1 clamped is compensated (reading R12).  Exact fractions."""
+    net = _post_net()
+    comp = net.composition.astype(np.float64)
+    o = w.SolverOpts()
+    on = oracle_mod.OracleNetwork(net, o)
+    y_in = np.array([0.30, 0.20, 0.05, 0.10, 0.40])
+    # final state: the a row lost 3e-3 atoms (a real violation, >> 1e-13), the b row drifted by 1e-15 (rounding level);
+    # nothing negative
+    y_f = y_in.copy(); y_f[0] -= 1e-3; y_f[2] -= 1e-3; y_f[1] += 1e-15
+    yo, st = on.finalize(y_f, y_in)
+    assert st == 0
+    # a row: the largest single-row species is `a` (0.299 > a2 = 0.049): it receives the 3e-3 missing atoms; b untouched
+    np.testing.assert_allclose(yo, [0.299 + 3e-3, 0.20 + 1e-15, 0.049, 0.10, 0.40], rtol=0, atol=6e-17)
+    assert abs((comp @ yo - comp @ y_in)[0]) < 3e-16 and (comp @ yo - comp @ y_in)[1] == pytest.approx(1e-15, rel=0.2)
+    # with a clamp in a drifting row the compensation is drift + clamp: ab = -0.01 clamped adds 0.01 a and 0.01 b,
+    # the a row additionally lost 2e-3 -> `a` gets +2e-3 - 0.01, b (row within tolerance) only -0.01
+    y_f2 = y_in.copy(); y_f2[0] -= 2e-3; y_f2[3] = -0.01
+    y_in2 = y_in.copy(); y_in2[3] = -0.01 + 0.0                     # the initial ab equals the final one: only `a` moved
+    yo2, st2 = on.finalize(y_f2, y_in2)
+    assert st2 == 2
+    np.testing.assert_allclose(yo2, [0.298 + 2e-3 - 0.01, 0.20 - 0.01, 0.05, 0.0, 0.40], rtol=0, atol=6e-17)
+    # cons_tol = inf: never more than the clamped amount (the round-1 reading); cons_tol = 0: always the full difference
+    o.cons_tol = float("inf")
+    yo3, _ = oracle_mod.OracleNetwork(net, o).finalize(y_f, y_in)
+    np.testing.assert_array_equal(yo3, y_f)
+    o.cons_tol = 0.0
+    yo4, _ = oracle_mod.OracleNetwork(net, o).finalize(y_f, y_in)
+    np.testing.assert_allclose(comp @ yo4, comp @ y_in, rtol=0, atol=3e-16)
+    assert yo4[1] == pytest.approx(0.20, abs=1e-16) and yo4[1] != y_f[1]
+    # through the step: a network whose Newton update does not conserve cannot be built (create validates N.dnu = 0), so
+    # the step-level check is that totals after a full step equal the input totals to rounding on every config
+    for idx, n in ((1, 64), (3, 24)):
+        netc, cells, opts = w.make_config(idx, n)
+        T, y, stc, stats, _ = oracle_mod.OracleNetwork(netc, opts).step(cells, n_threads=4)
+        Nm = netc.composition.astype(np.float64)
+        drift = np.abs((y - cells.y) @ Nm.T) / (np.abs(cells.y) @ np.abs(Nm).T)
+        assert drift.max() <= 1.0e-13
+
+
+def test_P11_stage_3_on_a_later_row_and_final_flags(oracle_mod):
+    """Stage 3 for the SECOND row of the matrix (the b row): elements a, b; species a, b, ab2, b2.  NEEDS_STAGE3 is
+    evaluated after all rows are processed: it is set iff some reservoir is still negative at the very end."""
+    net = H.tiny_network([[1, 0, 1, 0], [0, 1, 2, 2]], [((0, 1, 1), (2,), 1e-30, 0.0, 0.0, 0, -1)])   # a, b, ab2, b2
+    on = oracle_mod.OracleNetwork(net, w.SolverOpts())
+    comp = net.composition.astype(np.float64)
+    # b2 = -0.05 is clamped (adds 0.10 b); the b row's reservoir is the largest of {b = 0.01, b2 = 0}: b -> -0.09;
+    # stage 3 takes ab2 apart: 0.045 molecules give back 0.09 b and release 0.045 a into `a`
+    y = np.array([0.2, 0.01, 0.3, -0.05])
+    yo, st = on.finalize(y)
+    assert st == (2 | 128) and yo.min() >= 0.0
+    np.testing.assert_allclose(comp @ yo, comp @ y, rtol=0, atol=6e-17)
+    np.testing.assert_allclose(yo, [0.2 + 0.045, 0.0, 0.3 - 0.045, 0.0], rtol=0, atol=6e-17)
+    # not enough ab2: used up, b stays negative -> both bits
+    y2 = np.array([0.2, 0.01, 0.02, -0.05])
+    yo2, st2 = on.finalize(y2)
+    assert st2 == (2 | 64 | 128) and yo2[2] == 0.0 and yo2[1] == pytest.approx(-0.09 + 0.04, abs=1e-16)
+    np.testing.assert_allclose(comp @ yo2, comp @ y2, rtol=0, atol=6e-17)
 
 
 # ---- P12: the retry procedure (PAPER.md:218, reading R24) --------------------------------------------------------------

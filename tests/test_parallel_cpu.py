@@ -73,3 +73,29 @@ def test_two_ranks_sharded_equals_one_rank(tmp_path, oracle_mod):
         for k, v in stats1.items():
             assert int(o[f"s_{k}"]) == v                # summed counters of the shards = counters of the whole
     assert sum(int(o["l_n_newton"]) for o in outs) == stats1["n_newton"]
+
+
+def test_bench_starts_its_own_ranks_when_not_under_torchrun():
+    """`python bench.py --gpus 2` (no torchrun environment) must take the launcher path -- one process per GPU -- and not
+    silently run one rank: on this CPU-only box that path stops at the device count, with a message that names it."""
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE")}
+    env["CUDA_VISIBLE_DEVICES"] = ""
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--steps", "1", "--warmup", "1"],
+                       capture_output=True, text=True, env=env, timeout=300)
+    assert r.returncode != 0
+    assert "--gpus 2 asked for, 0 CUDA device(s) visible" in (r.stderr + r.stdout)
+
+
+def test_strong_scaling_shards_one_batch():
+    """bench.py --scaling strong: every rank draws the SAME full-size batch and keeps its block-cyclic share."""
+    net = w.make_network(2)
+    whole = w.make_cells(2, net, 10000, seed=w.BASE_SEED + 1002)
+    parts = [par.shard_cells(w.make_cells(2, net, 10000, seed=w.BASE_SEED + 1002), r, 4) for r in range(4)]
+    assert sum(p.n_cells for p in parts) == whole.n_cells
+    back = np.empty_like(whole.y)
+    for r, p in enumerate(parts):
+        back[par.shard_indices(whole.n_cells, r, 4)] = p.y
+    np.testing.assert_array_equal(back, whole.y)
