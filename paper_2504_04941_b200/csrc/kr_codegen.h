@@ -19,6 +19,11 @@ struct KrHostNet {
   std::vector<int> rprog_ptr, fac, tgt, emeta[4];       // streams: [0..1] kr_wpc.cuh layout (32 / 64 threads), [2..3] kr_row.cuh layout
   int n_entries = 0, elen[4] = {0, 0, 0, 0};
   std::vector<KrETerm> estream[4];
+  // balanced row program of kr_row.cuh (f rows and the T column): per group size (32 / 64 threads) a coalesced stream of
+  // (reaction | (dnu + 128) << 16, partial-sum slot or -1) words and the slot range of every species
+  std::vector<unsigned> rstream[2];
+  std::vector<int> rslot_ptr[2];
+  int rlen[2] = {0, 0}, n_rslots[2] = {0, 0};
 };
 
 namespace kr_codegen {

@@ -54,19 +54,21 @@ constexpr int oNN = oX + 8 * N;                         // [S+1] number densitie
 constexpr int oTH = oNN + 8 * (S + 1);                  // [3S] ghat, uhat, chat
 constexpr int oKF = oTH + 8 * 3 * S;                    // [R]
 constexpr int oKR = oKF + 8 * R;                        // [R]
-constexpr int oQ = oKR + 8 * R;                         // [R]  q_r
+constexpr int oQ = oKR + (KRR_ANY_REV ? 8 * R : 0);     // [R]  q_r (KR exists only when some reaction is reversible)
 constexpr int oDQT = oQ + 8 * R;                        // [R]  dq_r/dT (energy)
 constexpr int oQH = oDQT + (ENERGY ? 8 * R : 0);        // [R]  k_f P' - k_r P'' (third body)
 constexpr int oMT = oQH + (KRR_ANY_TB ? 8 * R : 0);     // [R]  M_r
 constexpr int oRED = oMT + (KRR_ANY_TB ? 8 * R : 0);    // [8 W + 4] reduction scratch, cell slot, scalars
 constexpr int oKEY = oRED + 8 * (8 * W + 4);            // int[2][W][2] pivot keys of the two warps (double buffered)
-constexpr int oUR = a16(oKEY + 4 * 2 * W * 2);          // [2][W][2 NC2] published pivot-row candidates (double buffered)
-constexpr int oJ = a16(oUR + 8 * 2 * W * 2 * NC2);      // [N][LDJ] J; column N holds f (the right-hand side is built from it)
+constexpr int NSLOT = KRR_NSLOT;                        // partial sums of the row program (host-built chunks)
+constexpr int oPART = a16(oKEY + 4 * 2 * W * 2);        // [NSLOT] partial f sums, then (energy) [NSLOT] partial T-column sums
+constexpr int oUR = a16(oPART + 8 * NSLOT * (ENERGY ? 2 : 1));   // [2][W][2 (NC2 + 1)] published pivot-row candidates + reciprocal (double buffered)
+constexpr int oJ = a16(oUR + 8 * 2 * W * 2 * (NC2 + 1));      // [N][LDJ] J; column N holds f (the right-hand side is built from it)
 constexpr int CELL_BYTES = a16(oJ + 8 * N * LDJ);
 
 #ifdef KRR_CELL_BYTES
 static_assert(CELL_BYTES == KRR_CELL_BYTES, "host and device disagree on the shared-memory layout");
-static_assert(oNN == 8 * KRR_I_NN && oKF == 8 * KRR_I_KF && oKR == 8 * KRR_I_KR, "host and device disagree on the vector offsets");
+static_assert(oNN == 8 * KRR_I_NN && oKF == 8 * KRR_I_KF && (!KRR_ANY_REV || oKR == 8 * KRR_I_KR), "host and device disagree on the vector offsets");
 static_assert(!KRR_ANY_TB || (oQH == 8 * KRR_I_QH && oMT == 8 * KRR_I_MT), "host and device disagree on the third-body offsets");
 static_assert(LDJ == KRR_LDJ, "host and device disagree on the row stride of J");
 #endif
@@ -224,9 +226,11 @@ __device__ __forceinline__ void reactions(const KrNetDev& n, const Cell& c, cons
           dlr = dlf - su * invT;
         }
       }
-      KF[r] = kf; KR[r] = kr;
+      KF[r] = kf;
+      if (KRR_ANY_REV) KR[r] = kr;
     } else {
-      kf = KF[r]; kr = KR[r];
+      kf = KF[r];
+      if (KRR_ANY_REV) kr = KR[r];
     }
     const double Pf = NN[f01.x] * NN[f01.y] * NN[f23.x];
     const double Pr = NN[f23.y] * NN[f45.x] * NN[f45.y];
@@ -248,20 +252,38 @@ __device__ __forceinline__ void reactions(const KrNetDev& n, const Cell& c, cons
   }
 }
 
-// ---- f rows (column N of J) and the T column of J when wantJ: thread <-> species row, gather in reaction order (eq. 15, eq. 20)
-__device__ __forceinline__ void rows(const KrNetDev& n, const Cell& c, const Grp& G, double invN, bool wantJ) {
-  double *Q = c.d(oQ), *J = c.d(oJ);
+// ---- f rows (column N of J) and the T column of J (eq. 15, eq. 20), in two passes.  Pass 1, thread <-> CHUNK of a species'
+// (reaction, dnu) list: the lists are cut into chunks of equal length on the host and dealt to the threads, so that the
+// row of an abundant species (three times the average length) does not hold up the group; the chunks reach each thread
+// as ONE coalesced stream of 8-byte words.  Pass 2, thread <-> species: the few partial sums of a species, in chunk
+// order (a fixed order: results do not depend on which thread summed what).
+__device__ __forceinline__ void row_partials(const KrNetDev& n, const Cell& c, const Grp& G) {
+  const double *Q = c.d(oQ), *DQT = c.d(oDQT);
+  double* PART = c.d(oPART);
+  const uint2* rs = n.rstream[W - 1] + G.gl;
+  const int len = n.rlen[W - 1];
+  double af = 0.0, at = 0.0;
+#pragma unroll 4
+  for (int i = 0; i < len; ++i) {
+    const uint2 t = __ldg(rs + i * GT);
+    const int r = (int)(t.x & 0xffffu);
+    const double dnu = (double)((int)(t.x >> 16) - 128);
+    af += dnu * Q[r];
+    if (ENERGY) at += dnu * DQT[r];
+    if ((int)t.y >= 0) {
+      PART[t.y] = af; af = 0.0;
+      if (ENERGY) { PART[NSLOT + t.y] = at; at = 0.0; }
+    }
+  }
+}
+__device__ __forceinline__ void row_combine(const KrNetDev& n, const Cell& c, const Grp& G, double invN, bool wantJ) {
+  const double* PART = c.d(oPART);
+  double* J = c.d(oJ);
+  const int* sp = n.rslot_ptr[W - 1];
   for (int s = G.gl; s < S; s += GT) {
     double ys = 0.0, jt = 0.0;
-    const int p1 = n.row_ptr[s + 1];
-#pragma unroll 4
-    for (int p = n.row_ptr[s]; p < p1; ++p) {
-      const int ent = __ldg(n.row_ent + p);
-      const int r = ent >> 8;
-      const double dnu = (double)((ent & 255) - 128);
-      ys += dnu * Q[r];
-      if (ENERGY) jt += dnu * c.d(oDQT)[r];
-    }
+    const int p1 = sp[s + 1];
+    for (int p = sp[s]; p < p1; ++p) { ys += PART[p]; if (ENERGY) jt += PART[NSLOT + p]; }
     J[s * LDJ + N] = ys * invN;
     if (ENERGY && wantJ) J[s * LDJ + S] = jt * invN;
   }
@@ -320,10 +342,12 @@ __device__ __forceinline__ void eval(const KrNetDev& n, const Cell& c, const Grp
   G.sync();
   const double heat_sum = red[0], heat_dT = red[1];
   const double invC = ENERGY ? krs_rcp(red[2]) : 1.0;
-  rows(n, c, G, invN, wantJ);
+  row_partials(n, c, G);
   if (wantJ) entries(n, c, G);
   G.sync();
-  if (ENERGY && wantJ) { trow(c, G, T, invC); G.sync(); }
+  row_combine(n, c, G, invN, wantJ);
+  if (ENERGY && wantJ) trow(c, G, T, invC);
+  G.sync();
   if (ENERGY) {
     double r2[3] = {0.0, 0.0, 0.0};
     for (int s = G.gl; s < S; s += GT) {
@@ -342,29 +366,169 @@ __device__ __forceinline__ void eval(const KrNetDev& n, const Cell& c, const Grp
 }
 
 // ---- step 7: elimination, one matrix row per lane ------------------------------------------------------------------
-// Pivot keys: the bits of |a| / scale; the warp-wide integer maximum of the high words, then, among the rows that share
-// the largest high word, of the low words with the row index folded into the 6 low bits -- together the 64-bit
-// lexicographic maximum: Algorithm 1's scaled pivot and its tie rule (smallest row) to 2^-46.  A used row carries a
-// negative scale and loses against every candidate.
-struct Cand { int hi; unsigned lo; };
-__device__ __forceinline__ Cand cand_of(double v, double sc, int row) {
-  const double t = fabs(v) * sc;
-  Cand k;
-  k.hi = __double2hiint(t);
-  k.lo = ((unsigned)__double2loint(t) | 63u) - (unsigned)row;
-  return k;
+// Pivot key of a row: the bit pattern of |a| / scale with the row index folded into its 6 low bits (63 - row), so that a
+// warp-wide integer maximum (REDUX on the high words, then on the low words of the rows that share the largest high
+// word) names the pivot row: Algorithm 1's scaled pivot, candidates closer than 2^-46 relative counting as tied, ties to
+// the smallest row (reading R14' of DESIGN.md).  A used row carries a negative scale: its key is negative and loses
+// against every candidate.
+#ifndef KRR_KEY64
+#define KRR_KEY64 1      // 0: 32-bit keys, one REDUX (measured: +5 % throughput, but candidates within 2^-14 tie, and on config 4
+#endif                   // that changed the accept / reject path of cells the oracle takes robustly) -- kept for experiments only
+#if KRR_KEY64
+// the whole bit pattern of |a| / scale with the row in the 6 low bits (ties to 2^-46), two REDUX
+typedef long long Key;
+__device__ __forceinline__ Key key_of(double v, double sc, int row) {
+  return (__double_as_longlong(fabs(v) * sc) | 63LL) - (long long)row;
 }
+__device__ __forceinline__ Key warp_max_key(Key k) {
+  const int hi = (int)(k >> 32);
+  const unsigned lo = (unsigned)k;
+  const int H = __reduce_max_sync(0xffffffffu, hi);
+  const unsigned L = __reduce_max_sync(0xffffffffu, (hi == H) ? lo : 0u);
+  return ((long long)H << 32) | (long long)L;
+}
+#else
+typedef int Key;
+__device__ __forceinline__ Key key_of(double v, double sc, int row) {
+  return (__double2hiint(fabs(v) * sc) | 63) - row;
+}
+__device__ __forceinline__ Key warp_max_key(Key k) { return __reduce_max_sync(0xffffffffu, k); }
+#endif
+
+// The elimination state of one thread; the column loop is a compile-time recursion (run<K>), so that every register
+// index is static whatever N is.
+//
+// The column loop is software-pipelined: as soon as the update of column k has produced the entries of column k + 1 the
+// search for pivot k + 1 is started (candidate keys, REDUX, a speculative reciprocal of every candidate), and the
+// remaining FMAs of update k are issued behind it, so that the latency of the search hides under the update.  The lane
+// that wins publishes its row together with its reciprocal.
+constexpr int XRD = XR > 0 ? XR : 1;
+constexpr int URS = NC2 + 1;                  // one published row: NC2 pairs + {reciprocal of its column-k entry, its key}
+
+struct Elim {
+  double2 a[NC2];                             // the lane's row of [J - I/h | G/h]
+  double xr[XRD][XQ];                         // spread rows: element j of spread row e in lane j % 32, slot j / 32
+  double sc, xsc[XRD];                        // > 0: 1 / scale of a candidate row; < 0: used (or no row)
+  double xk[XRD];                             // the spread rows' entries of the column being searched
+  double myrp, xrp[XRD];                      // reciprocal pivot of the column in which the row was the pivot row ...
+  int mycol, xcol[XRD];                       // ... and that column
+  Key kw;                                     // the warp's best key for the column being searched
+  double rk;                                  // speculative reciprocal of this lane's candidate
+  int gl, lane, wq;
+  double2* URb;
+  const Grp* G;
+
+  __device__ __forceinline__ double col(int k) const { return (k & 1) ? a[k >> 1].y : a[k >> 1].x; }
+
+  // candidate search for column KK on the rows as they stand: the warp's best key (REDUX), and the speculative
+  // reciprocal of this lane's candidate (overlaps the reduction; only the winner's is used)
+  template <int KK>
+  __device__ __forceinline__ void pick() {
+    const double ak = col(KK);
+    Key key = key_of(ak, sc, gl);
+#pragma unroll
+    for (int e = 0; e < XR; ++e) {             // element KK of a spread row sits in lane KK % 32: every lane gets it
+      xk[e] = __shfl_sync(0xffffffffu, xr[e][KK >> 5], KK & 31);
+      const Key kx = key_of(xk[e], xsc[e], NR + e);
+      key = (kx > key) ? kx : key;
+    }
+    kw = warp_max_key(key);
+    rk = krs_rcp(ak);
+  }
+  // publication of the warp's winner: its row from column KK on (every earlier update applied), the reciprocal of its
+  // column-KK entry and the key
+  template <int KK>
+  __device__ __forceinline__ void publish() {
+    constexpr int buf = KK & 1;
+    const int pw = (kw >= 0) ? (63 - (int)(kw & 63)) : -1;
+    double2* URw = URb + (buf * W + wq) * URS;
+    if (gl == pw) {
+#pragma unroll
+      for (int j = KK >> 1; j < NC2; ++j) URw[j] = a[j];
+      URw[NC2] = make_double2(rk, __longlong_as_double((long long)kw));
+    }
+#pragma unroll
+    for (int e = 0; e < XR; ++e)
+      if (pw == NR + e) {
+#pragma unroll
+        for (int q = 0; q < XQ; ++q)
+          if (lane + 32 * q < NC) reinterpret_cast<double*>(URw)[lane + 32 * q] = xr[e][q];
+        if (lane == 0) URw[NC2] = make_double2(krs_rcp(xk[e]), __longlong_as_double((long long)kw));
+      }
+    if (W > 1 && pw < 0 && lane == 0) URw[NC2] = make_double2(0.0, __longlong_as_double(-1LL));   // no candidate in this warp
+  }
+
+  template <int K>
+  __device__ __forceinline__ void column() {
+    constexpr int buf = K & 1, K2 = K >> 1;
+    // ---- the pivot row of column K: the warp's candidate, or the better of the two warps' candidates -------------------
+    Key kbest = kw;
+    const double2* URw = URb + (buf * W + wq) * URS;
+    double2 tail;
+    if (W > 1) {
+      G->sync();
+      const double2 t0 = URb[(buf * W + 0) * URS + NC2], t1 = URb[(buf * W + 1) * URS + NC2];
+      const Key k0 = (Key)__double_as_longlong(t0.y), k1 = (Key)__double_as_longlong(t1.y);
+      const bool second = k1 > k0;                           // keys carry the row: they are never equal unless both are -1
+      kbest = second ? k1 : k0;
+      tail = second ? t1 : t0;
+      URw = URb + (buf * W + (second ? 1 : 0)) * URS;
+    } else {
+      __syncwarp();
+      tail = URw[NC2];
+    }
+    const int p = (kbest >= 0) ? (63 - (int)(kbest & 63)) : -1;
+    // ---- broadcast read of the pivot row and its reciprocal, rank-1 update of the lane's row -----------------------------
+    const double rp = tail.x;
+    const bool mine = (gl == p);
+    const double l = mine ? 0.0 : -(col(K) * rp);          // the pivot row itself is not updated
+    if (mine) { sc = -1.0; mycol = K; myrp = rp; }
+    double xl[XRD];
+#pragma unroll
+    for (int e = 0; e < XR; ++e) {
+      const bool xmine = (p == NR + e);
+      xl[e] = xmine ? 0.0 : -(xk[e] * rp);
+      if (xmine) { xsc[e] = -1.0; xcol[e] = K; xrp[e] = rp; }
+    }
+    // column K + 1 first: its entries feed the next search
+    constexpr int J1 = (K & 1) ? K2 + 1 : K2;              // the pair that holds column K + 1
+    const double2 u1 = URw[J1];
+    if (K & 1) a[J1].x = fma(l, u1.x, a[J1].x);
+    else a[J1].y = fma(l, u1.y, a[J1].y);
+#pragma unroll
+    for (int e = 0; e < XR; ++e)
+#pragma unroll
+      for (int q = 0; q < XQ; ++q) {
+        const int j = lane + 32 * q;
+        if (j > K && j < NC) xr[e][q] = fma(xl[e], reinterpret_cast<const double*>(URw)[j], xr[e][q]);
+      }
+    // the search for pivot K + 1 is issued in front of the rest of update K; its winner publishes its row behind it
+    if constexpr (K + 1 < N) pick<K + 1>();
+    if (K & 1) a[J1].y = fma(l, u1.y, a[J1].y);
+#pragma unroll
+    for (int j = J1 + 1; j < NC2; ++j) {
+      const double2 u = URw[j];
+      a[j].x = fma(l, u.x, a[j].x); a[j].y = fma(l, u.y, a[j].y);
+    }
+    if constexpr (K + 1 < N) publish<K + 1>();
+  }
+
+  template <int K>
+  __device__ __forceinline__ void run() {
+    column<K>();
+    if constexpr (K + 1 < N) run<K + 1>();
+  }
+};
 
 // On success X holds the solution delta of (I - hJ) delta = -(U - UN - h f).  Uniform return value (false: zero row,
 // non-finite entry, no pivot or a pivot below 1e-300 in the units of I - hJ).
 __device__ __forceinline__ bool eliminate(const Cell& c, const Grp& G, double h) {
-  const int gl = G.gl, lane = gl & 31, wq = gl >> 5;
+  Elim E;
+  E.gl = G.gl; E.lane = G.gl & 31; E.wq = G.gl >> 5; E.G = &G;
+  const int gl = E.gl, lane = E.lane;
   double *U = c.d(oU), *UN = c.d(oUN), *X = c.d(oX), *J = c.d(oJ);
   const double invh = krs_rcp(h);
   const bool rin = gl < NR;
-  // ---- the lane's row of [J - I/h | G/h] -----------------------------------------------------------------------
-  double2 a[NC2];
-  double xr[XR > 0 ? XR : 1][XQ];             // spread rows: element j of spread row e in lane j % 32, slot j / 32
   {
     const double2* Jr = reinterpret_cast<const double2*>(J + (rin ? gl : 0) * LDJ);
     double d0 = 0.0;
@@ -379,134 +543,59 @@ __device__ __forceinline__ bool eliminate(const Cell& c, const Grp& G, double h)
     }
     __syncwarp();
 #pragma unroll
-    for (int j = 0; j < NC2; ++j) a[j] = rin ? Jr[j] : make_double2(0.0, 0.0);
+    for (int j = 0; j < NC2; ++j) E.a[j] = rin ? Jr[j] : make_double2(0.0, 0.0);
     if (rin) J[gl * LDJ + gl] = d0;           // J keeps its entries (structural zeros are never rewritten)
 #pragma unroll
     for (int e = 0; e < XR; ++e)
 #pragma unroll
       for (int q = 0; q < XQ; ++q) {
         const int j = lane + 32 * q;
-        xr[e][q] = (j < NC) ? J[(NR + e) * LDJ + j] : 0.0;
+        E.xr[e][q] = (j < NC) ? J[(NR + e) * LDJ + j] : 0.0;
       }
   }
-  // row scales (max-norm of the matrix part, Algorithm 1's implicit scaling); sc > 0: 1 / scale of a candidate row, < 0: used
+  // row scales (max-norm of the matrix part, Algorithm 1's implicit scaling)
   double big = 0.0;
-  bool fin = true;
 #pragma unroll
   for (int j = 0; j < NC2; ++j) {
-    if (2 * j < N) { const double ax = fabs(a[j].x); big = (ax > big) ? ax : big; fin = fin && (ax <= 1.7e308); }
-    if (2 * j + 1 < N) { const double ay = fabs(a[j].y); big = (ay > big) ? ay : big; fin = fin && (ay <= 1.7e308); }
+    if (2 * j < N) { const double ax = fabs(E.a[j].x); big = (ax > big || !(ax == ax)) ? ax : big; }
+    if (2 * j + 1 < N) { const double ay = fabs(E.a[j].y); big = (ay > big || !(ay == ay)) ? ay : big; }
   }
-  bool rows_ok = !rin || (fin && big > 0.0);
-  double sc = (rin && big > 0.0) ? krs_rcp(big) : -1.0;
-  double xsc[XR > 0 ? XR : 1];
+  bool rows_ok = !rin || (big > 0.0 && big <= 1.7e308);
+  E.sc = (rin && big > 0.0) ? krs_rcp(big) : -1.0;
 #pragma unroll
   for (int e = 0; e < XR; ++e) {
     double m = 0.0;
 #pragma unroll
     for (int q = 0; q < XQ; ++q)
-      if (lane + 32 * q < N) { const double ax = fabs(xr[e][q]); m = (ax > m || !(ax == ax)) ? ax : m; }
+      if (lane + 32 * q < N) { const double ax = fabs(E.xr[e][q]); m = (ax > m || !(ax == ax)) ? ax : m; }
     m = warp_max_nonneg(m);
     rows_ok = rows_ok && (m > 0.0) && (m <= 1.7e308);
-    xsc[e] = (m > 0.0) ? krs_rcp(m) : -1.0;
+    E.xsc[e] = (m > 0.0) ? krs_rcp(m) : -1.0;
   }
   rows_ok = G.all(rows_ok);
   if (!rows_ok) return false;
 
-  double* UR = c.d(oUR);
-  int* KEY = c.i(oKEY);
-  int mycol = -1;                             // the column in which this lane's row was the pivot row
-  double myrp = 0.0;                          // ... and the reciprocal of that pivot
-  int xcol[XR > 0 ? XR : 1];
-  double xrp[XR > 0 ? XR : 1];
+  E.URb = reinterpret_cast<double2*>(c.d(oUR));
+  E.mycol = -1; E.myrp = 0.0; E.kw = -1; E.rk = 0.0;
 #pragma unroll
-  for (int e = 0; e < XR; ++e) { xcol[e] = -1; xrp[e] = 0.0; }
-  bool fail = false;                          // uniform; no early exit from the column loop (keeps the warp converged)
-  const double pmin = 1e-300 * invh;          // |pivot| >= 1e-300 in the units of I - hJ
+  for (int e = 0; e < XRD; ++e) { E.xcol[e] = -1; E.xrp[e] = 0.0; E.xk[e] = 0.0; if (e >= XR) E.xsc[e] = -1.0; }
 
+  E.template pick<0>();
+  E.template publish<0>();
+  E.template run<0>();
+
+  // every row must have been a pivot row, with |pivot| >= 1e-300 in the units of I - hJ (|pivot'| >= 1e-300 / h here) and finite
+  const double rmax = 1e300 * h;
+  bool ok = !rin || (E.mycol >= 0 && fabs(E.myrp) <= rmax && fabs(E.myrp) > 0.0);
 #pragma unroll
-  for (int k = 0; k < N; ++k) {
-    const int buf = k & 1;
-    const double ak = (k & 1) ? a[k >> 1].y : a[k >> 1].x;
-    // ---- scaled pivot search -------------------------------------------------------------------------------------
-    Cand best = cand_of(ak, sc, gl);
-    double xk[XR > 0 ? XR : 1];
-#pragma unroll
-    for (int e = 0; e < XR; ++e) {             // the spread rows' candidates: element k sits in lane k % 32 -> every lane gets it
-      xk[e] = __shfl_sync(0xffffffffu, xr[e][k >> 5], k & 31);
-      const Cand x = cand_of(xk[e], xsc[e], NR + e);
-      if (x.hi > best.hi || (x.hi == best.hi && x.lo > best.lo)) best = x;
-    }
-    const int H = __reduce_max_sync(0xffffffffu, best.hi);
-    const unsigned Lw = __reduce_max_sync(0xffffffffu, (best.hi == H) ? best.lo : 0u);
-    int p = (H >= 0) ? (63 - (int)(Lw & 63u)) : -1;          // the warp's pivot row
-    double2* URw = reinterpret_cast<double2*>(UR) + (buf * W + wq) * NC2;
-    // ---- the lane that holds the candidate row writes it to shared memory (columns >= k, in pairs) -------------------
-    if (gl == p) {
-#pragma unroll
-      for (int j = k >> 1; j < NC2; ++j) URw[j] = a[j];
-    }
-#pragma unroll
-    for (int e = 0; e < XR; ++e)
-      if (p == NR + e) {
-#pragma unroll
-        for (int q = 0; q < XQ; ++q)
-          if (lane + 32 * q < NC) reinterpret_cast<double*>(URw)[lane + 32 * q] = xr[e][q];
-      }
-    if (W > 1) {                               // two warps: the better of the two candidates wins
-      if (lane == 0) { KEY[(buf * W + wq) * 2] = H; KEY[(buf * W + wq) * 2 + 1] = (int)Lw; }
-      G.sync();
-      const int H0 = KEY[(buf * W + 0) * 2], H1 = KEY[(buf * W + 1) * 2];
-      const unsigned L0 = (unsigned)KEY[(buf * W + 0) * 2 + 1], L1 = (unsigned)KEY[(buf * W + 1) * 2 + 1];
-      const bool second = (H1 > H0) || (H1 == H0 && L1 > L0);
-      const int Hw = second ? H1 : H0;
-      const unsigned Lg = second ? L1 : L0;
-      p = (Hw >= 0) ? (63 - (int)(Lg & 63u)) : -1;
-      URw = reinterpret_cast<double2*>(UR) + (buf * W + (second ? 1 : 0)) * NC2;
-    } else {
-      __syncwarp();
-    }
-    fail = fail || (p < 0);
-    // ---- broadcast read of the pivot row, reciprocal pivot, rank-1 update of the lane's row ---------------------------
-    double2 u[NC2];
-#pragma unroll
-    for (int j = k >> 1; j < NC2; ++j) u[j] = URw[j];
-    const double pv = (k & 1) ? u[k >> 1].y : u[k >> 1].x;
-    const bool pok = (fabs(pv) >= pmin) && (fabs(pv) <= 1.7e308);
-    fail = fail || !pok;
-    const double rp = krs_rcp(pok ? pv : 1.0);
-    const bool mine = (gl == p);
-    if (mine) { sc = -1.0; mycol = k; myrp = rp; }
-    if (!mine) {
-      const double l = -(ak * rp);
-      if (k & 1) {
-        // column k is the .y half of pair k >> 1: that pair is finished for this row
-      } else {
-        a[k >> 1].y = fma(l, u[k >> 1].y, a[k >> 1].y);
-      }
-#pragma unroll
-      for (int j = (k >> 1) + 1; j < NC2; ++j) { a[j].x = fma(l, u[j].x, a[j].x); a[j].y = fma(l, u[j].y, a[j].y); }
-    }
-#pragma unroll
-    for (int e = 0; e < XR; ++e) {
-      if (p == NR + e) { xsc[e] = -1.0; xcol[e] = k; xrp[e] = rp; }
-      else {
-        const double l = -(xk[e] * rp);
-#pragma unroll
-        for (int q = 0; q < XQ; ++q) {
-          const int j = lane + 32 * q;
-          if (j > k && j < NC) xr[e][q] = fma(l, reinterpret_cast<const double*>(URw)[j], xr[e][q]);
-        }
-      }
-    }
-  }
-  fail = !G.all(!fail);
-  if (fail) return false;
+  for (int e = 0; e < XR; ++e) ok = ok && (E.xcol[e] >= 0 && fabs(E.xrp[e]) <= rmax && fabs(E.xrp[e]) > 0.0);
+  ok = G.all(ok);
+  if (!ok) return false;
   // row p_k now holds x_k * pivot_k in its right-hand-side slot
-  if (rin && mycol >= 0) X[mycol] = ((N & 1) ? a[N >> 1].y : a[N >> 1].x) * myrp;
+  if (rin) X[E.mycol] = E.col(N) * E.myrp;
 #pragma unroll
   for (int e = 0; e < XR; ++e)
-    if (lane == (N & 31) && xcol[e] >= 0) X[xcol[e]] = xr[e][N >> 5] * xrp[e];
+    if (lane == (N & 31)) X[E.xcol[e]] = E.xr[e][N >> 5] * E.xrp[e];
   G.sync();
   return true;
 }

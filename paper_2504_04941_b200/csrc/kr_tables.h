@@ -77,6 +77,11 @@ struct KrNetDev {
   const KrETerm* estream[2];
   const int* emeta[2];
   int elen[2];
+  // row program of kr_row.cuh: step i of thread t reads rstream[i * GT + t] = {reaction | (dnu + 128) << 16, slot or -1};
+  // the partial sums of species s are the slots rslot_ptr[s] .. rslot_ptr[s + 1]
+  const uint2* rstream[2];
+  const int* rslot_ptr[2];
+  int rlen[2];
 };
 
 struct KrOptsDev {
