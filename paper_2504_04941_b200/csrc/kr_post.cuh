@@ -45,10 +45,11 @@ __device__ __forceinline__ int kr_post_argmax(const int* list, int lo, int hi, Y
 }
 
 // yin(s): abundance of species s at the start of the step (read-only); y(s): reference to its final abundance.
-template <class Yin, class Y>
+// MAXR: an upper bound of the number of conservation rows known at compile time (the network-specialised kernels pass E).
+template <int MAXR = KR_MAX_ROWS, class Yin, class Y>
 __device__ inline int kr_postprocess(const KrPostLists& L, double cons_tol, Yin yin, Y y) {
-  double full[KR_MAX_ROWS], clamp[KR_MAX_ROWS], scale[KR_MAX_ROWS];
-  int home[KR_MAX_ROWS];                 // packed res entry of the species that took the row's compensation, or -1
+  double full[MAXR], clamp[MAXR], scale[MAXR];
+  int home[MAXR];                        // packed res entry of the species that took the row's compensation, or -1
   int bits = 0;
   for (int nu = 0; nu < L.E; ++nu) { full[nu] = 0.0; clamp[nu] = 0.0; scale[nu] = 0.0; home[nu] = -1; }
 
@@ -116,26 +117,6 @@ __device__ inline int kr_postprocess(const KrPostLists& L, double cons_tol, Yin 
   for (int nu = 0; nu < L.E; ++nu)
     if (home[nu] >= 0 && y(kr_pk_index(home[nu])) < 0.0) bits |= KR_DST_NEEDS_STAGE3;
   return bits;
-}
-
-// Cheap screen used by the kernels that call the repair out of line: does this cell need it at all?  True when an
-// abundance is negative or a row's initial-minus-final total exceeds cons_tol x scale.
-template <class Yin, class Y>
-__device__ __forceinline__ bool kr_post_needed(const KrPostLists& L, double cons_tol, Yin yin, Y y) {
-  double full[KR_MAX_ROWS], scale[KR_MAX_ROWS];
-  for (int nu = 0; nu < L.E; ++nu) { full[nu] = 0.0; scale[nu] = 0.0; }
-  bool need = false;
-  for (int s = 0; s < L.S; ++s) {
-    const double before = yin(s), now = y(s);
-    need = need || (now < 0.0);
-    for (int i = L.sp_ptr[s]; i < L.sp_ptr[s + 1]; ++i) {
-      const int e = L.sp_ent[i], nu = kr_pk_index(e);
-      full[nu] += kr_pk_coef(e) * (before - now);
-      scale[nu] += fabs(kr_pk_coef(e) * before);
-    }
-  }
-  for (int nu = 0; nu < L.E; ++nu) need = need || (fabs(full[nu]) > cons_tol * scale[nu]);
-  return need;
 }
 
 // the view of the table-driven kernels

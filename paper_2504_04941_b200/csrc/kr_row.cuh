@@ -766,7 +766,7 @@ kr_row_kernel(const KrNetDev n, const KrOptsDev o, const KrStepArgs a) {
     }
     // ---- step 9: finalise (PAPER.md:212-216 stages 1-3, kr_post.cuh; serial in thread 0, once per cell) + layout-out ----
     if (o.finalize && G.gl == 0) {
-      st |= kr_postprocess(kr_post_lists(n), o.cons_tol, [&](int s) { return a.y[cell * S + s]; }, [&](int s) -> double& { return UN[s]; });
+      st |= kr_postprocess<E>(kr_post_lists(n), o.cons_tol, [&](int s) { return a.y[cell * S + s]; }, [&](int s) -> double& { return UN[s]; });
       if (a.status) a.status[cell] = st;
     } else if (G.gl == 0 && a.status) {
       a.status[cell] = st;

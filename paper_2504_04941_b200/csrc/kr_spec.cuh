@@ -299,7 +299,7 @@ __device__ __forceinline__ KrPostLists krs_post_lists() {
                      KrNet::post_cmp_ptr, KrNet::post_cmp_ent, KrNet::signed_row};
 }
 __device__ __noinline__ int krs_post(double* un0, const double* yin, double cons_tol) {
-  return kr_postprocess(krs_post_lists(), cons_tol, [&](int s) { return yin[s]; }, [&](int s) -> double& { return un0[s * KRS_BLOCK]; });
+  return kr_postprocess<KrNet::E>(krs_post_lists(), cons_tol, [&](int s) { return yin[s]; }, [&](int s) -> double& { return un0[s * KRS_BLOCK]; });
 }
 
 enum { KRS_FETCH = 0, KRS_RUN = 1, KRS_DONE = 2 };
