@@ -373,7 +373,7 @@ __device__ __forceinline__ void eval(const KrNetDev& n, const Cell& c, const Grp
 // against every candidate.
 #ifndef KRR_KEY64
 #define KRR_KEY64 1      // 0: 32-bit keys, one REDUX (measured: +5 % throughput, but candidates within 2^-14 tie, and on config 4
-#endif                   // that changed the accept / reject path of cells the oracle takes robustly) -- kept for experiments only
+#endif                   // that changed the accept / reject path of cells whose decisions have wide margins) -- kept for experiments only
 #if KRR_KEY64
 // the whole bit pattern of |a| / scale with the row in the 6 low bits (ties to 2^-46), two REDUX
 typedef long long Key;
