@@ -246,6 +246,7 @@ def bench_one(idx: int, mode_name: str, args, ctx) -> dict:
         ms = gn.last_mixed_stats()
         mixed_stats = {"refinements_per_newton": ms["n_refine"] / max(stats["n_newton"], 1),
                        "fp64_fallback_cell_fraction": ms["n_fp64_cells"] / max(n_cells, 1),
+                       "discarded_newton_per_cell": ms["n_discarded_newton"] / max(n_cells, 1),
                        "fp64_kernel": "fp64 warp-per-cell kernel on the listed cells (second launch)"}
     flops_step = F.step_flops(net, stats)
     kern_ms = float(np.mean(ms_each))                     # this rank's step

@@ -131,6 +131,10 @@ int kr_set_stream(kr_network *net, void *cuda_stream);
 /* Override the mapping picked from N: mapping = KR_MAP_*, threads_per_cell = 0 (auto) or a multiple
  * of 32 for KR_MAP_WARP (32) / KR_MAP_CTA (64..256).  KR_EUNSUPPORTED when N does not fit it. */
 int kr_network_set_mapping(kr_network *net, int32_t mapping, int32_t threads_per_cell);
+/* Test and study hooks (the defaults are what the library measures best): stiffest_first -1 = automatic (a cost pass and a
+ * sort before warp-per-cell launches of several waves), 0 = always index order, 1 = as automatic; host_chunks 0 = automatic,
+ * 1..8 = that many chunks in kr_thermochem_step_host.  Results do not depend on either (cells are independent). */
+int kr_network_set_tuning(kr_network *net, int32_t stiffest_first, int32_t host_chunks);
 /* Query: N (unknowns per cell), mapping in use, threads per cell, dynamic shared memory per block. */
 int kr_network_info(const kr_network *net, int32_t *n_unknowns, int32_t *mapping, int32_t *threads_per_cell,
                     int32_t *smem_bytes);
@@ -188,9 +192,11 @@ int kr_network_row_compile(const kr_network_desc *desc, int32_t warps_per_cell, 
                            void *cubin, int64_t cubin_cap);
 
 /* Mixed precision only, counters of the last step call summed over cells: refinement passes (fp64 residual + fp32
- * replay), and cells whose fp32 factorisation could not be refined and that were redone by the fp64 kernel (status bit
- * KR_ST_FP64_FALLBACK).  Synchronises the device.  HOST pointers, either may be NULL. */
-int kr_last_mixed_stats(kr_network *net, int64_t *n_refine, int64_t *n_fp64_cells);
+ * replay), cells whose fp32 factorisation could not be refined and that were redone by the fp64 kernel (status bit
+ * KR_ST_FP64_FALLBACK), and the Newton iterations of those abandoned fp32 attempts (they are NOT part of kr_step_stats:
+ * the statistics count the work of the attempt that produced the result).  Synchronises the stream of the last step
+ * call.  HOST pointers, each may be NULL. */
+int kr_last_mixed_stats(kr_network *net, int64_t *n_refine, int64_t *n_fp64_cells, int64_t *n_discarded_newton);
 
 /* Number of kernel launches the last step call on this handle queued (for bench.py's gpu_launches). */
 int kr_last_launch_count(const kr_network *net);

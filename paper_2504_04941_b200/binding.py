@@ -24,7 +24,7 @@ ST_REJECTED_ONCE, ST_CLAMPED_NEG, ST_FP64_FALLBACK, ST_FAILED_REVERTED, ST_T_CLA
 
 EXPORTS = [
     "kr_network_create", "kr_network_destroy", "kr_default_opts", "kr_network_set_options",
-    "kr_network_get_options", "kr_set_stream", "kr_network_set_mapping", "kr_network_info",
+    "kr_network_get_options", "kr_set_stream", "kr_network_set_mapping", "kr_network_set_tuning", "kr_network_info",
     "kr_network_kernel_desc", "kr_network_spec_source", "kr_network_spec_compile", "kr_network_wpc_compile", "kr_network_row_compile", "kr_last_mixed_stats", "kr_thermochem_step", "kr_thermochem_step_ex", "kr_thermochem_step_host", "kr_last_launch_count",
     "kr_layout_cell_to_soa", "kr_layout_soa_to_cell", "kr_math_probe", "kr_measure_fp64_peak", "kr_last_error", "kr_version",
 ]
@@ -103,7 +103,8 @@ def load() -> C.CDLL:
                                            C.c_void_p, C.c_int64]
     lib.kr_network_wpc_compile.argtypes = [C.POINTER(NetworkDesc), C.c_int, C.c_int32, C.POINTER(C.c_int64), C.c_char_p, C.c_int64,
                                            vp, C.c_int64]
-    lib.kr_last_mixed_stats.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+    lib.kr_last_mixed_stats.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+    lib.kr_network_set_tuning.argtypes = [vp, C.c_int32, C.c_int32]
     lib.kr_layout_cell_to_soa.argtypes = [vp, vp, C.c_int64, C.c_int32, vp]
     lib.kr_layout_soa_to_cell.argtypes = [vp, vp, C.c_int64, C.c_int32, vp]
     lib.kr_measure_fp64_peak.argtypes = [C.c_int32, _dp]
@@ -236,18 +237,7 @@ class Network:
 
     def __init__(self, net, opts=None):
         lib = load()
-        self._keep = dict(
-            elem_mass=_f64(net.elem_mass), composition=_i32(net.composition),
-            reac_idx=_i32(net.reac_idx), reac_nu=_i32(net.reac_nu), prod_idx=_i32(net.prod_idx),
-            prod_nu=_i32(net.prod_nu), A=_f64(net.A), beta=_f64(net.beta), Ea=_f64(net.Ea_over_k),
-            flags=_i32(net.flags), aux_index=_i32(net.aux_index), tb_eff=_f64(net.tb_eff), q_ext=_f64(net.q_ext),
-            nasa_lo=_f64(net.nasa_lo), nasa_hi=_f64(net.nasa_hi), T_mid=_f64(net.T_mid))
-        k = self._keep
-        d = NetworkDesc(net.n_elem, net.n_species, net.n_reac, _d(k["elem_mass"]), _i(k["composition"]),
-                        _i(k["reac_idx"]), _i(k["reac_nu"]), _i(k["prod_idx"]), _i(k["prod_nu"]),
-                        _d(k["A"]), _d(k["beta"]), _d(k["Ea"]), _i(k["flags"]), _i(k["aux_index"]),
-                        _d(k["tb_eff"]), _d(k["q_ext"]), _d(k["nasa_lo"]), _d(k["nasa_hi"]), _d(k["T_mid"]),
-                        float(net.T_lo), float(net.T_hi), int(net.energy_equation))
+        d, self._keep = make_desc(net)
         h = C.c_void_p()
         self._h = None
         _check(lib.kr_network_create(C.byref(d), C.byref(h)))
@@ -286,6 +276,9 @@ class Network:
     def set_mapping(self, mapping: int, threads_per_cell: int = 0) -> None:
         _check(load().kr_network_set_mapping(self._h, int(mapping), int(threads_per_cell)))
 
+    def set_tuning(self, stiffest_first: int = -1, host_chunks: int = 0) -> None:
+        _check(load().kr_network_set_tuning(self._h, int(stiffest_first), int(host_chunks)))
+
     def info(self) -> dict:
         a, b, c, d = C.c_int32(), C.c_int32(), C.c_int32(), C.c_int32()
         _check(load().kr_network_info(self._h, C.byref(a), C.byref(b), C.byref(c), C.byref(d)))
@@ -300,9 +293,9 @@ class Network:
         return int(load().kr_last_launch_count(self._h))
 
     def last_mixed_stats(self) -> dict:
-        a, b = C.c_int64(), C.c_int64()
-        _check(load().kr_last_mixed_stats(self._h, C.byref(a), C.byref(b)))
-        return {"n_refine": int(a.value), "n_fp64_cells": int(b.value)}
+        a, b, c = C.c_int64(), C.c_int64(), C.c_int64()
+        _check(load().kr_last_mixed_stats(self._h, C.byref(a), C.byref(b), C.byref(c)))
+        return {"n_refine": int(a.value), "n_fp64_cells": int(b.value), "n_discarded_newton": int(c.value)}
 
     # -- the step -----------------------------------------------------------------------------
     def thermochem_step(self, n_cells: int, rho, T, y, dt: float, precision_mode: int = KR_FP64) -> None:

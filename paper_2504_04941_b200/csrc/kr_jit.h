@@ -1,7 +1,10 @@
 // kr_jit.h -- host side: run-time compilation (NVRTC, sm_100a) and loading of the network-specialised kernel.
 // NVRTC is dlopen'ed (no link-time dependency), the driver entry points come from cudaGetDriverEntryPoint, so
-// the library still loads on a machine without a GPU.  Compiled cubins are cached in the process and on disk
-// ($KR_CACHE_DIR, default /tmp/kratos_chem_cache) under a hash of the exact source and options.
+// the library still loads on a machine without a GPU.  Compiled cubins are cached in the process (per CUDA context) and
+// on disk under a hash of the exact source and options: $KR_CACHE_DIR, else $XDG_CACHE_HOME/kratos_chem, else
+// ~/.cache/kratos_chem, else /tmp/kratos_chem_cache_<uid>; the directory is created 0700 and must belong to the calling
+// user, every file carries a length + checksum header that is verified before the image is used (a file that fails is
+// ignored and recompiled).
 #pragma once
 #include <cuda.h>
 #include <cuda_runtime.h>
@@ -12,6 +15,7 @@
 #include <cstdint>
 #include <cstdio>
 #include <cstdlib>
+#include <cstring>
 #include <map>
 #include <mutex>
 #include <string>
@@ -34,6 +38,7 @@ struct Driver {
                            void**, void**) = nullptr;
   CUresult (*OccupancyMaxActiveBlocksPerMultiprocessor)(int*, CUfunction, int, size_t) = nullptr;
   CUresult (*GetErrorString)(CUresult, const char**) = nullptr;
+  CUresult (*CtxGetCurrent)(CUcontext*) = nullptr;
   bool ok = false;
 };
 
@@ -53,6 +58,7 @@ inline Driver& driver() {
     ok &= get("cuLaunchKernel", (void**)&d.LaunchKernel);
     ok &= get("cuOccupancyMaxActiveBlocksPerMultiprocessor", (void**)&d.OccupancyMaxActiveBlocksPerMultiprocessor);
     ok &= get("cuGetErrorString", (void**)&d.GetErrorString);
+    ok &= get("cuCtxGetCurrent", (void**)&d.CtxGetCurrent);
     cudaGetLastError();
     d.ok = ok;
   });
@@ -109,12 +115,20 @@ inline uint64_t fnv1a(const std::string& s, uint64_t h = 1469598103934665603ull)
   return h;
 }
 
+// "" when no directory that belongs to the calling user (and to nobody else) can be had: the disk cache is then off
 inline std::string cache_dir() {
-  const char* e = getenv("KR_CACHE_DIR");
-  std::string d = e ? e : "/tmp/kratos_chem_cache";
-  mkdir(d.c_str(), 0777);
+  std::string d;
+  if (const char* e = getenv("KR_CACHE_DIR")) d = e;
+  else if (const char* x = getenv("XDG_CACHE_HOME")) { d = std::string(x); mkdir(d.c_str(), 0700); d += "/kratos_chem"; }
+  else if (const char* h = getenv("HOME")) { d = std::string(h) + "/.cache"; mkdir(d.c_str(), 0700); d += "/kratos_chem"; }
+  else d = "/tmp/kratos_chem_cache_" + std::to_string((unsigned)getuid());
+  mkdir(d.c_str(), 0700);
+  struct stat st;
+  if (stat(d.c_str(), &st) != 0 || !S_ISDIR(st.st_mode) || st.st_uid != getuid() || (st.st_mode & 022)) return "";
   return d;
 }
+
+struct CacheHeader { char magic[8]; uint64_t length, checksum; };
 
 struct Header { const char* name; const char* text; };
 
@@ -132,15 +146,16 @@ inline std::vector<char> compile(const std::string& source, const std::vector<He
   key += "|sm_100a|c++17|lineinfo|nvrtc" + std::to_string(vmaj) + "." + std::to_string(vmin);
   char name[64];
   snprintf(name, sizeof name, "%016llx%016llx", (unsigned long long)fnv1a(key), (unsigned long long)fnv1a(key, 88172645463325252ull));
-  const std::string path = cache_dir() + "/" + name + ".cubin";
-  if (!getenv("KR_NO_DISK_CACHE")) {
+  const std::string dir = getenv("KR_NO_DISK_CACHE") ? std::string() : cache_dir();
+  const std::string path = dir + "/" + name + ".krc";
+  if (!dir.empty()) {
     if (FILE* f = fopen(path.c_str(), "rb")) {
-      fseek(f, 0, SEEK_END);
-      const long sz = ftell(f);
-      fseek(f, 0, SEEK_SET);
-      if (sz > 0) {
-        cubin.resize(size_t(sz));
-        if (fread(cubin.data(), 1, size_t(sz), f) != size_t(sz)) cubin.clear();
+      CacheHeader hd;
+      if (fread(&hd, sizeof hd, 1, f) == 1 && std::string(hd.magic, 8) == "KRCUBIN1" && hd.length > 0 && hd.length < (1ull << 28)) {
+        cubin.resize(size_t(hd.length));
+        if (fread(cubin.data(), 1, cubin.size(), f) != cubin.size() ||
+            fnv1a(std::string(cubin.begin(), cubin.end())) != hd.checksum)
+          cubin.clear();                       // truncated or altered: recompile
       }
       fclose(f);
       if (!cubin.empty()) { if (from_cache) *from_cache = true; return cubin; }
@@ -168,10 +183,13 @@ inline std::vector<char> compile(const std::string& source, const std::vector<He
     }
   }
   n.DestroyProgram(&prog);
-  if (!cubin.empty() && !getenv("KR_NO_DISK_CACHE")) {
+  if (!cubin.empty() && !dir.empty()) {
     const std::string tmp = path + "." + std::to_string(getpid()) + ".tmp";
     if (FILE* f = fopen(tmp.c_str(), "wb")) {
-      const bool ok = fwrite(cubin.data(), 1, cubin.size(), f) == cubin.size();
+      CacheHeader hd;
+      memcpy(hd.magic, "KRCUBIN1", 8);
+      hd.length = cubin.size(); hd.checksum = fnv1a(std::string(cubin.begin(), cubin.end()));
+      const bool ok = fwrite(&hd, sizeof hd, 1, f) == 1 && fwrite(cubin.data(), 1, cubin.size(), f) == cubin.size();
       fclose(f);
       if (ok) rename(tmp.c_str(), path.c_str()); else remove(tmp.c_str());
     }
@@ -179,17 +197,19 @@ inline std::vector<char> compile(const std::string& source, const std::vector<He
   return cubin;
 }
 
-// in-process cache: cubin hash -> loaded kernel (modules live until process exit)
+// in-process cache: (CUDA context, cubin hash) -> loaded kernel (modules live until process exit)
 inline bool load(const std::vector<char>& cubin, const char* entry, Kernel& out, std::string& err) {
   static std::mutex mu;
-  static std::map<uint64_t, Kernel> loaded;
+  static std::map<std::pair<uintptr_t, uint64_t>, Kernel> loaded;
   Driver& d = driver();
   if (!d.ok) { err = "CUDA driver entry points unavailable"; return false; }
-  const uint64_t key = fnv1a(std::string(cubin.begin(), cubin.end()));
+  cudaFree(0);                                    // make sure the primary context of the current device is current
+  CUcontext ctx = nullptr;
+  if (d.CtxGetCurrent) d.CtxGetCurrent(&ctx);
+  const std::pair<uintptr_t, uint64_t> key(reinterpret_cast<uintptr_t>(ctx), fnv1a(std::string(cubin.begin(), cubin.end())));
   std::lock_guard<std::mutex> lk(mu);
   auto it = loaded.find(key);
   if (it != loaded.end()) { out = it->second; return true; }
-  cudaFree(0);                                    // make sure the primary context is current
   Kernel k;
   CUresult r = d.ModuleLoadData(&k.mod, cubin.data());
   if (r == CUDA_SUCCESS) r = d.ModuleGetFunction(&k.fn, k.mod, entry);

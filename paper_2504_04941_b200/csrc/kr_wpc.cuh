@@ -701,6 +701,7 @@ kr_wpc_kernel(const KrNetDev n, const KrOptsDev o, const KrStepArgs a) {
   double *U = c.d(oU), *UN = c.d(oUN), *F = c.d(oF), *X = c.d(oX);
 
   unsigned long long c_acc = 0, c_rej = 0, c_newton = 0, c_rate = 0, c_failed = 0, c_ref = 0;   // thread 0 of the group
+  unsigned long long c_disc = 0;        // Newton iterations of fp32 attempts that were handed to the fp64 kernel (not algorithmic work)
 
   for (;;) {
     if (G.gl == 0) {
@@ -714,6 +715,7 @@ kr_wpc_kernel(const KrNetDev n, const KrOptsDev o, const KrStepArgs a) {
     if (cell >= a.n_cells) break;
 
     // ---- step 1: layout-in, clamp, first sub-step -------------------------------------------------
+    const unsigned long long s_newton = c_newton, s_rate = c_rate, s_ref = c_ref;     // counters at the start of this cell
     int st = a.list ? a.list_flag : 0;
     double Tc = a.T[cell];
     if (Tc < n.T_lo) { Tc = n.T_lo; st |= KR_DST_T_CLAMPED; }
@@ -852,6 +854,8 @@ kr_wpc_kernel(const KrNetDev n, const KrOptsDev o, const KrStepArgs a) {
       continue;
     }
     if (handoff) {            // the caller's buffers were never written: the fp64 kernel redoes this cell from its input
+      c_disc += c_newton - s_newton;                              // the abandoned attempt is not counted as work of the step
+      c_newton = s_newton; c_rate = s_rate; c_ref = s_ref;
       if (G.gl == 0) a.retry_list[atomicAdd(a.retry_count, 1ull)] = cell;
       G.sync();
       continue;
@@ -879,5 +883,6 @@ kr_wpc_kernel(const KrNetDev n, const KrOptsDev o, const KrStepArgs a) {
     atomicAdd(a.stats + 0, c_acc); atomicAdd(a.stats + 1, c_rej); atomicAdd(a.stats + 2, c_newton);
     atomicAdd(a.stats + 3, c_newton); atomicAdd(a.stats + 4, c_rate); atomicAdd(a.stats + 5, c_failed);
     if (c_ref) atomicAdd(a.stats + 6, c_ref);
+    if (c_disc) atomicAdd(a.stats + 13, c_disc);
   }
 }

@@ -30,9 +30,11 @@ def B():
     return binding
 
 
-def run_gpu(B, net, cells, opts, mode=0, mapping=None, tpc=0, host=False):
+def run_gpu(B, net, cells, opts, mode=0, mapping=None, tpc=0, host=False, index_order=False):
     import torch
     gn = B.Network(net, opts)
+    if index_order:
+        gn.set_tuning(stiffest_first=0)
     if mapping is not None:
         gn.set_mapping(mapping, tpc)
     n = cells.n_cells
@@ -149,15 +151,14 @@ def test_results_are_deterministic(B, idx, n, mode):
         assert stats == runs[0][3]
 
 
-def test_stiffest_first_scheduling_changes_nothing(B, monkeypatch):
+def test_stiffest_first_scheduling_changes_nothing(B):
     """The register-tile launches of several waves run a cost pass, sort the cells by their first sub-step and walk the
     sorted list; cells are independent, so results, status and counters must be
     bit-identical to the index-order run, and the extra launches must be counted."""
     net, cells, opts = w.make_config(3, 9000)                  # > 4 waves of 11 cells x 148 SMs
     T1, y1, s1, st1, g1 = run_gpu(B, net, cells, opts)
     assert g1.last_launch_count() == 9                         # cost pass, iota, 6 radix-sort kernels, solve
-    monkeypatch.setenv("KR_NO_LPT", "1")
-    T0, y0, s0, st0, g0 = run_gpu(B, net, cells, opts)
+    T0, y0, s0, st0, g0 = run_gpu(B, net, cells, opts, index_order=True)
     assert g0.last_launch_count() == 1
     np.testing.assert_array_equal(y1, y0)
     np.testing.assert_array_equal(T1, T0)
@@ -165,7 +166,7 @@ def test_stiffest_first_scheduling_changes_nothing(B, monkeypatch):
     assert st1 == st0
 
 
-def test_retry_with_stiffest_first_scheduling(B, monkeypatch):
+def test_retry_with_stiffest_first_scheduling(B):
     """The retry pass behind a list-driven first launch (several waves -> cost pass + sort): every cell is written exactly
     once, and the result equals the index-order run bit for bit."""
     net, cells, opts = w.make_config(3, 9000)
@@ -173,8 +174,7 @@ def test_retry_with_stiffest_first_scheduling(B, monkeypatch):
     T1, y1, s1, st1, g1 = run_gpu(B, net, cells, opts)
     assert (s1 >= 0).all() and ((s1 & 256) != 0).sum() > 1000          # run_gpu pre-fills the status with -1
     assert g1.last_launch_count() == 10
-    monkeypatch.setenv("KR_NO_LPT", "1")
-    T0, y0, s0, st0, g0 = run_gpu(B, net, cells, opts)
+    T0, y0, s0, st0, g0 = run_gpu(B, net, cells, opts, index_order=True)
     np.testing.assert_array_equal(y1, y0)
     np.testing.assert_array_equal(s1, s0)
     assert st1 == st0 and g0.last_launch_count() == 2
@@ -293,14 +293,14 @@ def test_host_variant_is_bit_identical_to_device_variant(B):
 
 
 @pytest.mark.parametrize("idx,n,chunks", [(2, 5003, 3), (1, 2049, 4), (3, 301, 8)])
-def test_pipelined_host_variant_is_bit_identical(B, monkeypatch, idx, n, chunks):
+def test_pipelined_host_variant_is_bit_identical(B, idx, n, chunks):
     """kr_thermochem_step_host cuts large batches into chunks and overlaps copy-in, step and copy-out on three streams
     (forced here on a small ragged batch): same bits as the device call, status and aux rows in the right places."""
     import torch
     net, cells, opts = w.make_config(idx, n)
     Td, yd, sd, _, _ = run_gpu(B, net, cells, opts)
-    monkeypatch.setenv("KR_HOST_CHUNKS", str(chunks))
     gn = B.Network(net, opts)
+    gn.set_tuning(host_chunks=chunks)
     pin = lambda a: torch.tensor(a).pin_memory()
     T = pin(cells.T); y = pin(cells.y); st = torch.full((n,), -1, dtype=torch.int32).pin_memory()
     rho = pin(cells.rho); aux = None if cells.aux is None else pin(cells.aux)
