@@ -515,3 +515,46 @@ def make_config(idx: int, n_cells: Optional[int] = None, fixed_newton: int = 0,
     net = make_network(idx)
     cells = make_cells(idx, net, n_cells, seed)
     return net, cells, default_opts(idx, fixed_newton)
+
+
+# --------------------------------------------------------------------------
+# species advection (NEXT-2: PAPER.md section 2.1, test of section 4.1) -- inputs only, no method arithmetic
+# --------------------------------------------------------------------------
+
+def advection_test_case(n_zones: int = 128, table=None):
+    """The four-species test of PAPER.md:400-417: returns (composition [2, 4], x_centres, y [n_zones, 4], rho, dx).
+    `table` is the parsed tests/golden/paper_eq33.txt (rows of left, right, slope, atoms of A, atoms of B); the defaults
+    are the same printed values."""
+    if table is None:
+        table = [(0.49, 0.05, 0.2, 1, 0), (0.20, 0.40, -0.1, 2, 0), (0.01, 0.05, 0.0, 1, 1), (0.09, 0.05, 0.0, 0, 1)]
+    dx = 1.0 / n_zones
+    x = -0.5 + dx * (np.arange(n_zones) + 0.5)
+    y = np.stack([l * (x < 0) + r * (x > 0) + k * x for l, r, k, _, _ in table], axis=1)
+    comp = np.array([[t[3] for t in table], [t[4] for t in table]], np.int32)
+    return comp, x, np.ascontiguousarray(y), np.ones(n_zones), dx
+
+
+def make_advection_batch(n_species: int, n_elem: int, n_cells: int, seed: int = BASE_SEED + 2000):
+    """Seeded synthetic 1-D field for the advection kernel's parity and bandwidth runs: random species compositions
+    (the first n_elem species are atoms), abundances with smooth waves, jumps and flat stretches, density and velocity
+    fields of both signs.  Returns (composition [E, S], y [n_cells, S], rho [n_cells], mass_flux [n_cells])."""
+    rng = np.random.default_rng(seed)
+    comp = np.zeros((n_elem, n_species), np.int32)
+    for s in range(n_species):
+        if s < n_elem:
+            comp[s, s] = 1
+        else:
+            k = rng.integers(1, min(3, n_elem) + 1)
+            for e in rng.choice(n_elem, size=k, replace=False):
+                comp[e, s] = rng.integers(1, 4)
+    xi = np.linspace(0.0, 1.0, n_cells, endpoint=False)
+    y = np.empty((n_cells, n_species))
+    for s in range(n_species):
+        wave = 0.5 + 0.4 * np.sin(2 * np.pi * (rng.integers(1, 9) * xi + rng.random()))
+        jump = np.where((xi > rng.random()) ^ (xi > rng.random()), rng.random(), 0.0)
+        flat = np.where(np.sin(2 * np.pi * rng.integers(1, 5) * xi) > 0.3, 1.0, 0.0)
+        y[:, s] = (wave * flat + jump + 1e-3) * 10.0 ** rng.uniform(-6, 0)
+    rho = 1.0 + 0.5 * np.sin(2 * np.pi * 3 * xi + 1.0)
+    vel = np.sin(2 * np.pi * 2 * xi + 0.3) + 0.2
+    flux = np.where(vel > 0, np.roll(rho, 1), rho) * vel
+    return comp, np.ascontiguousarray(y), rho, flux
