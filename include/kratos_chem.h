@@ -215,6 +215,30 @@ int kr_math_probe(const double *x, double *rcp, double *ex, int64_t n, void *cud
  * the achieved TFLOP/s in *tflops (host) measured with CUDA events over n_iter inner iterations. */
 int kr_measure_fp64_peak(int32_t n_iter, double *tflops);
 
+/* ---- Species reconstruction and advection (section 2.1, eqs. 1-14) -------------------------
+ * The step that precedes the chemistry step in the paper's cycle: the abundances y (the chemistry step's variable, y = n m_u / rho
+ * = m_u x of eq. 1) are advected with the mass fluxes of the hydrodynamics, F^s = y_{i-1/2} F^rho (eq. 1), the interface state
+ * being the upwind cell's (eq. 6, donor cell), its piecewise-linear extrapolation with the modified van Leer limiter (eqs. 9-12),
+ * or that extrapolation with the correction projected onto the stoichiometric space, P = V V^T from the SVD of the
+ * element-species matrix (eqs. 7, 8, 13), which keeps every element total of the interface state equal to the upwind cell's. */
+typedef struct kr_recon kr_recon;
+enum { KR_RECON_SCHEME_DONOR = 0, KR_RECON_SCHEME_PLM = 1, KR_RECON_SCHEME_PLM_PROJECTED = 2 };
+/* composition: HOST [n_elem * n_species] row-major N_{nu,s}.  Builds P on the host (one-sided Jacobi SVD) and
+ * uploads it when a CUDA device is present (without one the handle only serves kr_recon_projector). */
+int kr_recon_create(int32_t n_elem, int32_t n_species, const int32_t *composition, kr_recon **out);
+void kr_recon_destroy(kr_recon *r);
+/* P: HOST [n_species * n_species] row-major, filled; rank (HOST, may be NULL) receives the rank of the composition matrix. */
+int kr_recon_projector(const kr_recon *r, double *P, int32_t *rank);
+/* One forward-Euler stage of the conservative update on a uniform 1-D grid (step (3) of PAPER.md:40), DEVICE pointers:
+ *   y [n_cells * S] cell-major, rho [n_cells], mass_flux: periodic != 0 -> [n_cells], mass_flux[i] = F^rho through the LEFT face
+ *   of cell i (the right face of the last cell is the left face of the first); periodic == 0 -> [n_cells + 1], zero-gradient
+ *   ghost cells at both ends.  rho_out = wa rho0 + wb (rho - dt_over_dx dF^rho), (rho y)_out likewise, y_out = (rho y)_out /
+ *   rho_out; y0 / rho0 NULL -> plain stage (wa, wb ignored as 0, 1).  y_out [n_cells * S] must not alias y; rho_out [n_cells] may
+ *   be NULL.  scheme = KR_RECON_SCHEME_*.  Asynchronous on cuda_stream.  KR_EINVAL on bad arguments, KR_ECUDA without a device. */
+int kr_advect_species_1d(kr_recon *r, int64_t n_cells, const double *y, const double *rho, const double *mass_flux,
+                         double dt_over_dx, double dx, int32_t scheme, int32_t periodic, double wa, double wb,
+                         const double *y0, const double *rho0, double *y_out, double *rho_out, void *cuda_stream);
+
 const char *kr_last_error(void);
 const char *kr_version(void);
 

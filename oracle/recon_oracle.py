@@ -21,7 +21,7 @@ and backward slopes a, b and geometric factors c_f, c_b:  phi = a b (c_f b + c_b
 when a b > 0, else 0, with c_f = (<xi>_{i+1} - <xi>_i) / (xi_{i+1/2} - <xi>_i), c_b = (<xi>_i - <xi>_{i-1}) /
 (<xi>_i - xi_{i-1/2}) (both 2 on a uniform grid, where phi is the harmonic mean 2ab/(a+b)).  R26 the time integrator of
 the test is not stated: the step here is ONE forward-Euler stage with optional convex-combination weights, so that the
-driver can run SSP-RK2.  R27 x^s = n^s / rho is carried as y^s = n^s m_u / rho, the chemistry step's variable.
+driver can run SSP-RK2.  R28 open ends use zero-gradient ghost cells.  R27 x^s = n^s / rho is carried as y^s = n^s m_u / rho, the chemistry step's variable.
 """
 from __future__ import annotations
 
@@ -74,8 +74,8 @@ def interface_states(y: np.ndarray, mass_flux: np.ndarray, dx: float, scheme: in
     d = cell_corrections(y, dx, scheme, P, periodic)
     if periodic:
         y_left = np.roll(y + d, 1, axis=0)         # cell i - 1 seen from its right face
-    else:
-        y_left = np.vstack([(y + d)[:1], (y + d)[:-1]])
+    else:                                          # open end: a zero-gradient ghost cell (its own correction is 0)
+        y_left = np.vstack([y[:1], (y + d)[:-1]])
     y_right = y - d                                # cell i seen from its left face
     up = (np.asarray(mass_flux) > 0.0)[:, None]
     return np.where(up, y_left, y_right)
@@ -96,7 +96,7 @@ def advect_stage(y, rho, mass_flux, dt_over_dx, dx, scheme, P, periodic=True, wa
         yr = np.roll(yl, -1, axis=0)
     else:                                          # open right end: the state at the last face
         d = cell_corrections(y, dx, scheme, P, periodic)
-        last = np.where(f[n] > 0.0, (y + d)[-1], (y - d)[-1])
+        last = np.where(f[n] > 0.0, (y + d)[-1], y[-1])          # ghost cell beyond the right end
         yr = np.vstack([yl[1:], last[None, :]])
     rho_new = rho - dt_over_dx * (f_right - f_left)
     u_new = rho[:, None] * y - dt_over_dx * (yr * f_right[:, None] - yl * f_left[:, None])

@@ -27,6 +27,7 @@ EXPORTS = [
     "kr_network_get_options", "kr_set_stream", "kr_network_set_mapping", "kr_network_set_tuning", "kr_network_info",
     "kr_network_kernel_desc", "kr_network_spec_source", "kr_network_spec_compile", "kr_network_wpc_compile", "kr_network_row_compile", "kr_last_mixed_stats", "kr_thermochem_step", "kr_thermochem_step_ex", "kr_thermochem_step_host", "kr_last_launch_count",
     "kr_layout_cell_to_soa", "kr_layout_soa_to_cell", "kr_math_probe", "kr_measure_fp64_peak", "kr_last_error", "kr_version",
+    "kr_recon_create", "kr_recon_destroy", "kr_recon_projector", "kr_advect_species_1d",
 ]
 
 _dp = C.POINTER(C.c_double)
@@ -109,6 +110,12 @@ def load() -> C.CDLL:
     lib.kr_layout_soa_to_cell.argtypes = [vp, vp, C.c_int64, C.c_int32, vp]
     lib.kr_measure_fp64_peak.argtypes = [C.c_int32, _dp]
     lib.kr_math_probe.argtypes = [vp, vp, vp, C.c_int64, vp]
+    lib.kr_recon_create.argtypes = [C.c_int32, C.c_int32, _ip, C.POINTER(vp)]
+    lib.kr_recon_destroy.argtypes = [vp]
+    lib.kr_recon_destroy.restype = None
+    lib.kr_recon_projector.argtypes = [vp, _dp, _ip]
+    lib.kr_advect_species_1d.argtypes = [vp, C.c_int64, vp, vp, vp, C.c_double, C.c_double, C.c_int32, C.c_int32, C.c_double,
+                                         C.c_double, vp, vp, vp, vp, vp]
     lib.kr_last_error.restype = C.c_char_p
     lib.kr_version.restype = C.c_char_p
     _lib = lib
@@ -334,3 +341,37 @@ def layout_cell_to_soa(y_cell, y_soa, n_cells: int, S: int, stream: int = 0) -> 
 
 def layout_soa_to_cell(y_soa, y_cell, n_cells: int, S: int, stream: int = 0) -> None:
     _check(load().kr_layout_soa_to_cell(_ptr(y_soa), _ptr(y_cell), int(n_cells), int(S), C.c_void_p(stream or None)))
+
+
+class Recon:
+    """kr_recon handle: the stoichiometric projector of a composition matrix and the species advection stage
+    (section 2.1).  Argument marshalling only."""
+
+    SCHEME_DONOR, SCHEME_PLM, SCHEME_PLM_PROJECTED = 0, 1, 2
+
+    def __init__(self, composition):
+        comp = _i32(composition)
+        self.E, self.S = int(comp.shape[0]), int(comp.shape[1])
+        h = C.c_void_p()
+        _check(load().kr_recon_create(self.E, self.S, _i(comp), C.byref(h)))
+        self._h = h
+
+    def __del__(self):
+        try:
+            if getattr(self, "_h", None):
+                load().kr_recon_destroy(self._h)
+                self._h = None
+        except Exception:
+            pass
+
+    def projector(self):
+        P = np.zeros((self.S, self.S))
+        rank = C.c_int32()
+        _check(load().kr_recon_projector(self._h, _d(P), C.byref(rank)))
+        return P, int(rank.value)
+
+    def advect_species_1d(self, n_cells, y, rho, mass_flux, dt_over_dx, dx, scheme, periodic, y_out, rho_out=None,
+                          wa=0.0, wb=1.0, y0=None, rho0=None, stream=None) -> None:
+        _check(load().kr_advect_species_1d(self._h, int(n_cells), _ptr(y), _ptr(rho), _ptr(mass_flux), float(dt_over_dx), float(dx),
+                                           int(scheme), int(bool(periodic)), float(wa), float(wb), _ptr(y0), _ptr(rho0),
+                                           _ptr(y_out), _ptr(rho_out), stream))

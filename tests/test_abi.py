@@ -128,3 +128,16 @@ def test_binding_has_no_cpu_fallback():
     for f in os.listdir(os.path.join(ROOT, "paper_2504_04941_b200", "csrc")):
         assert "oracle" not in open(os.path.join(ROOT, "paper_2504_04941_b200", "csrc", f)).read().lower().replace(
             "the oracle's", "").replace("oracle/", ""), f
+
+
+@pytest.mark.parametrize("idx", [0, 1, 2, 3, 4])
+def test_recon_projector_host_svd(B, idx):
+    """kr_recon_create builds P = V V^T (eq. 8) on the host with its own one-sided Jacobi SVD -- no GPU
+    needed: against the textbook projector onto null(N), and the rank of N."""
+    N = w.make_network(idx).composition.astype(np.float64)
+    P, rank = B.Recon(N.astype(np.int32)).projector()
+    ref = np.eye(N.shape[1]) - N.T @ np.linalg.solve(N @ N.T, N)
+    assert rank == np.linalg.matrix_rank(N)
+    assert np.abs(P - ref).max() < 1e-13 and np.abs(N @ P).max() < 1e-13 and np.abs(P @ P - P).max() < 1e-13
+    P2, rank2 = B.Recon(np.vstack([N, N[:1]]).astype(np.int32)).projector()       # rank-deficient input
+    assert rank2 == rank and np.abs(P2 - P).max() < 1e-13
