@@ -316,6 +316,54 @@ def bench_one(idx: int, mode_name: str, args, ctx) -> dict:
     }
 
 
+def hbm_peak():
+    """(GB/s, source): MEASURED_PEAKS.json's copy bandwidth (driver-written), else the profiling guide's fallback."""
+    try:
+        return float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs"
+    except Exception:
+        return 6650.0, "fallback 6.65 TB/s of /opt/skills/guides/B200_PROFILING.md (MEASURED_PEAKS.json absent)"
+
+
+def bench_advection(args, ctx) -> dict:
+    """one stage of kr_advect_species_1d (projected PLM, eqs. 9-14) on a seeded synthetic
+    1-D field with config 1's composition matrix; HBM-bound: algorithmic bytes 16 S + 24 per cell (read y, rho, mass flux;
+    write y, rho) over the event-timed launch, against the measured copy bandwidth."""
+    import torch
+    from paper_2504_04941_b200 import binding as B
+    dev = ctx["dev"]
+    n = args.advect_cells
+    comp = w.make_network(1).composition
+    S = comp.shape[1]
+    _, yb, rb, fb = w.make_advection_batch(S, comp.shape[0], 1 << 16, seed=w.BASE_SEED + 2001)
+    reps = (n + yb.shape[0] - 1) // yb.shape[0]
+    y = torch.tensor(yb, device=dev).repeat(reps, 1)[:n].contiguous()
+    rho = torch.tensor(rb, device=dev).repeat(reps)[:n].contiguous()
+    flux = torch.tensor(fb, device=dev).repeat(reps)[:n].contiguous()
+    y_out = torch.empty_like(y); rho_out = torch.empty_like(rho)
+    rc = B.Recon(comp)
+    stream = torch.cuda.current_stream()
+    dx, lam = 1.0 / n, 0.2
+    run = lambda: rc.advect_species_1d(n, y, rho, flux, lam, dx, B.Recon.SCHEME_PLM_PROJECTED, True, y_out, rho_out,
+                                       stream=stream.cuda_stream)
+    for _ in range(3):
+        run()
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for a, b in ev:
+        ctx["flush"].zero_()
+        a.record(stream); run(); b.record(stream)
+    torch.cuda.synchronize()
+    ms = float(np.mean([a.elapsed_time(b) for a, b in ev]))
+    bytes_launch = float(n) * (16 * S + 24)
+    peak, src = hbm_peak()
+    gbs = bytes_launch / (ms * 1e-3) / 1e9
+    return {"workload": f"advection_1d_S{S}_projected_plm", "dtype": "f64", "cells": n, "value": n / (ms * 1e-3), "unit": "cell-updates/s",
+            "ms_per_launch": ms, "gpu_launches": args.steps,
+            "roofline": {"bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak, "traffic": None,
+                         "traffic_note": TRAFFIC_NOTE, "peak_source": src, "bytes_per_launch": bytes_launch},
+            "note": "the step before the chemistry step in the paper's cycle (PAPER.md section 2.1); input larger than L2 and L2 flushed between launches"}
+
+
 def worker(args, rank: int, local_rank: int, world: int) -> None:
     import torch
     import torch.distributed as dist
@@ -332,6 +380,10 @@ def worker(args, rank: int, local_rank: int, world: int) -> None:
     ctx = dict(rank=rank, local_rank=local_rank, world=world, dev=dev,
                flush=torch.empty(256 << 20, dtype=torch.uint8, device=dev),       # > 126 MB L2
                peak_tf=B.measure_fp64_peak(8192))
+    if args.advection_only:
+        if rank == 0:
+            print(json.dumps({"next": {"advection": bench_advection(args, ctx)}}), flush=True)
+        return
     if args.config is not None:
         runs = [(args.config, args.mode)]
     elif world > 1 and not args.all_configs:
@@ -342,6 +394,9 @@ def worker(args, rank: int, local_rank: int, world: int) -> None:
     for idx, mode_name in runs:
         results.append(bench_one(idx, mode_name, args, ctx))
         torch.cuda.empty_cache()
+    advection = None
+    if rank == 0 and world == 1 and args.config is None and not args.no_advection:
+        advection = bench_advection(args, ctx)
     if rank == 0:
         head = next((r for r, (i, m) in zip(results, runs) if i == HEADLINE and m == "fp64"), results[0])
         line = dict(head)
@@ -357,6 +412,8 @@ def worker(args, rank: int, local_rank: int, world: int) -> None:
                                 "kernel": r["config"]["kernel"], "cells_per_gpu": r["config"]["cells_per_gpu"],
                                 "notes": r["config"]["notes"]} for r in results]
             line["gpu_launches"] = int(sum(r["gpu_launches"] for r in results))
+        if advection is not None:
+            line["next"] = {"advection": advection}
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
@@ -385,6 +442,9 @@ def main() -> None:
     ap.add_argument("--cpu-seconds", type=float, default=10.0, help="budget of the oracle timing per config")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-advection", action="store_true", help="skip the NEXT-2 advection-stage bandwidth measurement")
+    ap.add_argument("--advect-cells", type=int, default=1 << 24)
+    ap.add_argument("--advection-only", action="store_true", help="measure only the NEXT-2 advection stage (profiling runs)")
     args = ap.parse_args()
     under_launcher = "RANK" in os.environ and "WORLD_SIZE" in os.environ
     rank = int(os.environ.get("RANK", "0"))

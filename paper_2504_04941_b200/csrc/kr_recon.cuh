@@ -10,6 +10,7 @@
 // (thread <-> (cell, species)), projected with the S x S matrix P held in shared memory (S FMAs per value, all operands
 // on chip), and the update of the tile is written back coalesced.  No atomics, fixed summation order.
 #pragma once
+#include "kr_math.cuh"
 
 #define KR_RECON_DONOR 0
 #define KR_RECON_PLM 1
@@ -31,11 +32,14 @@ struct KrAdvectArgs {
   double* rho_out;
 };
 
-// modified van Leer limiter (eq. 12, reading R25) for a uniform grid: c_f = c_b = 2
-__device__ __forceinline__ double kr_limited_slope(double a, double b) {
-  const double prod = a * b;
-  const double den = b * b + 2.0 * prod + a * a;
-  return (prod > 0.0) ? prod * (2.0 * b + 2.0 * a) / den : 0.0;
+// Limited half-difference of eq. 10 on a uniform grid: with the forward and backward differences dp = y_{i+1} - y_i and
+// dm = y_i - y_{i-1}, the modified van Leer slope (eq. 12, reading R25: c_f = c_b = 2, the harmonic mean 2ab/(a+b) of the
+// difference quotients a = dp / dx, b = dm / dx) times dx / 2 is dp dm / (dp + dm): dx cancels, one reciprocal per value.
+// (FP64 divides are DFMA sequences on this chip and this kernel must stay HBM-bound: krs_rcp is 1 ulp in 5 instructions.)
+__device__ __forceinline__ double kr_limited_half_difference(double dp, double dm) {
+  const double prod = dp * dm;
+  const double sum = dp + dm;
+  return (prod > 0.0) ? prod * krs_rcp(sum) : 0.0;
 }
 
 __device__ __forceinline__ long long kr_wrap(long long c, long long n, int periodic) {
@@ -43,71 +47,234 @@ __device__ __forceinline__ long long kr_wrap(long long c, long long n, int perio
   return c < 0 ? 0 : (c >= n ? n - 1 : c);
 }
 
-__global__ void __launch_bounds__(256) kr_advect_kernel(const KrAdvectArgs a) {
+// thread <-> (cell, species) without a division per element: element i = cl * S + s advances by the block size
+struct KrElemWalk {
+  int cl, s, dq, dr, S;
+  __device__ __forceinline__ KrElemWalk(int tid, int nthr, int S_) : cl(tid / S_), s(tid % S_), dq(nthr / S_), dr(nthr % S_), S(S_) {}
+  __device__ __forceinline__ void next() { cl += dq; s += dr; if (s >= S) { s -= S; ++cl; } }
+};
+
+__global__ void __launch_bounds__(128) kr_advect_kernel(const KrAdvectArgs a) {
   extern __shared__ double kr_rs[];
   const int S = a.S, T = a.T, LDP = S | 1;
   double* sP = kr_rs;                          // [S][LDP]
   double* sy = sP + S * LDP;                   // [T + 4][S]   cells c0 - 2 .. c0 + T + 1
   double* sg = sy + (T + 4) * S;               // [T + 2][S]   limited half-differences of cells c0 - 1 .. c0 + T
   double* sd = sg + (T + 2) * S;               // [T + 2][S]   ... projected
+  double* sr = sd + (T + 2) * S;               // [T][4]       per cell: rho, left flux, right flux, 1 / rho_out
   const long long c0 = (long long)blockIdx.x * T;
   const int nt = (int)min((long long)T, a.n_cells - c0);
   const int tid = threadIdx.x, nthr = blockDim.x;
 
   if (a.scheme == KR_RECON_PLM_PROJECTED)
     for (int i = tid; i < S * S; i += nthr) sP[(i / S) * LDP + (i % S)] = a.P[i];
-  // stage the tile + halo (coalesced: consecutive threads read consecutive doubles)
-  for (int i = tid; i < (nt + 4) * S; i += nthr) {
-    const int cl = i / S, s = i - cl * S;
-    const long long c = kr_wrap(c0 - 2 + cl, a.n_cells, a.periodic);
-    sy[i] = a.y[c * S + s];
+  // stage the tile + halo (coalesced: consecutive threads read consecutive doubles; the interior is one contiguous range)
+  {
+    const long long e0 = (c0 - 2) * S, n_el = a.n_cells * S;
+    const int tot = (nt + 4) * S;
+    if (c0 >= 2 && c0 + nt + 2 <= a.n_cells) {
+      for (int i = tid; i < tot; i += nthr) sy[i] = a.y[e0 + i];
+    } else {
+      for (KrElemWalk w(tid, nthr, S); w.cl < nt + 4; w.next())
+        sy[w.cl * S + w.s] = a.y[kr_wrap(c0 - 2 + w.cl, a.n_cells, a.periodic) * S + w.s];
+    }
+    (void)n_el;
+  }
+  // per-cell scalars: density, the two face fluxes, the reciprocal of the new density (one per cell, not one per value)
+  for (int cl = tid; cl < nt; cl += nthr) {
+    const long long c = c0 + cl;
+    const double fl = a.flux[c];
+    const double fr = a.periodic ? a.flux[(c + 1 == a.n_cells) ? 0 : c + 1] : a.flux[c + 1];
+    const double rho = a.rho[c];
+    double rn = rho - a.lambda * (fr - fl);
+    if (a.y0) rn = a.wa * a.rho0[c] + a.wb * rn;
+    sr[4 * cl] = rho; sr[4 * cl + 1] = fl; sr[4 * cl + 2] = fr; sr[4 * cl + 3] = krs_rcp(rn);
+    if (a.rho_out) a.rho_out[c] = rn;
   }
   __syncthreads();
-  // limited half-differences d = phi(a, b) dx / 2 of cells c0 - 1 .. c0 + nt (eqs. 10-12)
+  // limited half-differences of cells c0 - 1 .. c0 + nt (eqs. 10-12); open ends: the halo rows hold copies of the end cell
+  // (zero-gradient ghost cells), whose own difference is then 0
   if (a.scheme != KR_RECON_DONOR) {
-    const double inv_dx = 1.0 / a.dx, half = 0.5 * a.dx;
-    for (int i = tid; i < (nt + 2) * S; i += nthr) {
-      const int cl = i / S, s = i - cl * S;                    // cell c0 - 1 + cl  <->  sy row cl + 1
-      // open ends: the halo rows hold copies of the end cell (zero-gradient ghost cells), whose own difference is then 0
-      const double yc = sy[(cl + 1) * S + s], ym = sy[cl * S + s], yp = sy[(cl + 2) * S + s];
-      const double fa = (yp - yc) * inv_dx, fb = (yc - ym) * inv_dx;
-      sg[i] = kr_limited_slope(fa, fb) * half;
+    const int tot = (nt + 2) * S;
+    for (int i = tid; i < tot; i += nthr) {                    // element i of sg <-> element i + S of sy
+      const double yc = sy[i + S];
+      sg[i] = kr_limited_half_difference(sy[i + 2 * S] - yc, yc - sy[i]);
     }
     __syncthreads();
     if (a.scheme == KR_RECON_PLM_PROJECTED) {                  // eq. 13: d^s <- sum_r P^s_r d^r
-      for (int i = tid; i < (nt + 2) * S; i += nthr) {
-        const int cl = i / S, s = i - cl * S;
-        const double* g = sg + cl * S;
-        const double* p = sP + s * LDP;
+      for (KrElemWalk w(tid, nthr, S); w.cl < nt + 2; w.next()) {
+        const double* g = sg + w.cl * S;
+        const double* p = sP + w.s * LDP;
         double acc = 0.0;
         for (int r = 0; r < S; ++r) acc += p[r] * g[r];
-        sd[i] = acc;
+        sd[w.cl * S + w.s] = acc;
       }
     } else {
-      for (int i = tid; i < (nt + 2) * S; i += nthr) sd[i] = sg[i];
+      for (int i = tid; i < tot; i += nthr) sd[i] = sg[i];
     }
   } else {
     for (int i = tid; i < (nt + 2) * S; i += nthr) sd[i] = 0.0;
   }
   __syncthreads();
   // conservative update of the tile (eq. 1, eq. 14, step 3 of PAPER.md:40)
-  for (int i = tid; i < nt * S; i += nthr) {
-    const int cl = i / S, s = i - cl * S;                      // cell c = c0 + cl: sy row cl + 2, sd row cl + 1
-    const long long c = c0 + cl;
-    const double fl = a.flux[c];
-    const double fr = a.periodic ? a.flux[(c + 1 == a.n_cells) ? 0 : c + 1] : a.flux[c + 1];
-    const double yc = sy[(cl + 2) * S + s], dc = sd[(cl + 1) * S + s];
-    const double yl = (fl > 0.0) ? sy[(cl + 1) * S + s] + sd[cl * S + s] : yc - dc;
-    const double yr = (fr > 0.0) ? yc + dc : sy[(cl + 3) * S + s] - sd[(cl + 2) * S + s];
-    const double rho = a.rho[c];
-    double rn = rho - a.lambda * (fr - fl);
+  for (KrElemWalk w(tid, nthr, S); w.cl < nt; w.next()) {
+    const int i = w.cl * S + w.s;                              // cell c0 + cl: sy row cl + 2, sd row cl + 1
+    const double rho = sr[4 * w.cl], fl = sr[4 * w.cl + 1], fr = sr[4 * w.cl + 2], rinv = sr[4 * w.cl + 3];
+    const double yc = sy[i + 2 * S], dc = sd[i + S];
+    const double yl = (fl > 0.0) ? sy[i + S] + sd[i] : yc - dc;
+    const double yr = (fr > 0.0) ? yc + dc : sy[i + 3 * S] - sd[i + 2 * S];
     double un = rho * yc - a.lambda * (yr * fr - yl * fl);
-    if (a.y0) {
-      const double r0 = a.rho0[c];
-      rn = a.wa * r0 + a.wb * rn;
-      un = a.wa * r0 * a.y0[c * S + s] + a.wb * un;
-    }
-    a.y_out[c * S + s] = un / rn;
-    if (s == 0 && a.rho_out) a.rho_out[c] = rn;
+    const long long e = (c0 + w.cl) * S + w.s;
+    if (a.y0) un = a.wa * a.rho0[c0 + w.cl] * a.y0[e] + a.wb * un;
+    a.y_out[e] = un * rinv;
   }
+}
+
+
+// ---- the same stage for S <= KR_RECON_SMAX species, S a compile-time constant: thread <-> CELL --------------------------
+// The generic kernel above spends ~300 instructions per value on index arithmetic, shared-memory operands and loop
+// control, which makes it issue-bound at a quarter of the HBM rate.  Here a thread keeps the S values of its cell in
+// registers, every loop over species is unrolled, and P travels in the kernel's parameter block: parameters live in the
+// constant bank, so each of the S^2 products of eq. 13 is ONE DFMA with a constant-bank operand -- no load, no index.
+#define KR_RECON_SMAX 16
+
+template <int S>
+struct KrAdvectArgsP {
+  KrAdvectArgs a;
+  double P[S * S];
+};
+
+__device__ __forceinline__ void kr_cp_async8(double* smem_dst, const double* gmem_src) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void kr_cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void kr_cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+// Persistent blocks walk the tiles with a stride of gridDim.x; the abundances of the NEXT tile are already on their way
+// into the second staging buffer (cp.async) while the current tile is limited, projected and updated, so that the HBM
+// reads overlap the arithmetic instead of alternating with it.
+template <int S>
+struct KrAdvectTile { static constexpr int T = (S <= 10) ? 128 : 64; };   // 48 KiB of static shared memory
+
+template <int S>
+__global__ void __launch_bounds__(KrAdvectTile<S>::T) kr_advect_cell_kernel(const KrAdvectArgsP<S> ap) {
+  constexpr int T = KrAdvectTile<S>::T, LDY = S | 1; // cells per tile = threads per block; padded row: conflict-free 64-bit accesses
+  const KrAdvectArgs& a = ap.a;
+  __shared__ double sybuf[2][(T + 4) * LDY];         // cells c0 - 2 .. c0 + T + 1, double buffered
+  __shared__ double sd[(T + 2) * LDY];               // corrections of cells c0 - 1 .. c0 + T; later the results of the tile
+  const int tid = threadIdx.x;
+  const long long n_tiles = (a.n_cells + T - 1) / T;
+
+  auto stage = [&](long long tile, double* sy) {      // asynchronous, coalesced copy of tile + halo into sy
+    const long long c0 = tile * T;
+    const int nt = (int)min((long long)T, a.n_cells - c0);
+    if (c0 >= 2 && c0 + nt + 2 <= a.n_cells) {
+      const double* src = a.y + (c0 - 2) * S;
+      if (LDY == S) { for (int i = tid; i < (nt + 4) * S; i += T) kr_cp_async8(sy + i, src + i); }
+      else { for (int i = tid; i < (nt + 4) * S; i += T) kr_cp_async8(sy + (i / S) * LDY + (i % S), src + i); }
+    } else {
+      for (int i = tid; i < (nt + 4) * S; i += T) {
+        const int cl = i / S, s = i % S;
+        kr_cp_async8(sy + cl * LDY + s, a.y + kr_wrap(c0 - 2 + cl, a.n_cells, a.periodic) * S + s);
+      }
+    }
+    kr_cp_async_commit();
+  };
+
+  int buf = 0;
+  if ((long long)blockIdx.x < n_tiles) stage(blockIdx.x, sybuf[0]);
+  for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, buf ^= 1) {
+    const double* sy = sybuf[buf];
+    const long long c0 = tile * T;
+    const int nt = (int)min((long long)T, a.n_cells - c0);
+    kr_cp_async_wait_all();
+    __syncthreads();                                  // the tile is in sy; everybody is done with the other buffer and with sd
+    if (tile + gridDim.x < n_tiles) stage(tile + gridDim.x, sybuf[buf ^ 1]);
+    // the cell's scalars are requested now, so that their latency hides under the corrections
+    const int cl = tid;
+    double fl = 0.0, fr = 0.0, rho = 1.0, r0 = 0.0;
+    if (cl < nt) {
+      const long long c = c0 + cl;
+      fl = a.flux[c];
+      fr = a.periodic ? a.flux[(c + 1 == a.n_cells) ? 0 : c + 1] : a.flux[c + 1];
+      rho = a.rho[c];
+      if (a.y0) r0 = a.rho0[c];
+    }
+    // corrections of cells c0 - 1 .. c0 + nt: limited half-differences (eqs. 10-12), projected (eq. 13)
+    for (int cl = tid; cl < nt + 2; cl += T) {
+      double g[S];
+      if (a.scheme == KR_RECON_DONOR) {
+#pragma unroll
+        for (int s = 0; s < S; ++s) g[s] = 0.0;
+      } else {
+#pragma unroll
+        for (int s = 0; s < S; ++s) {
+          const double yc = sy[(cl + 1) * LDY + s];
+          g[s] = kr_limited_half_difference(sy[(cl + 2) * LDY + s] - yc, yc - sy[cl * LDY + s]);
+        }
+      }
+      if (a.scheme == KR_RECON_PLM_PROJECTED) {
+#pragma unroll
+        for (int s = 0; s < S; ++s) {
+          double acc = 0.0;
+#pragma unroll
+          for (int r = 0; r < S; ++r) acc += ap.P[s * S + r] * g[r];
+          sd[cl * LDY + s] = acc;
+        }
+      } else {
+#pragma unroll
+        for (int s = 0; s < S; ++s) sd[cl * LDY + s] = g[s];
+      }
+    }
+    __syncthreads();
+    // conservative update of the tile (eq. 1, eq. 14, step 3 of PAPER.md:40); results staged for a coalesced write
+    double out[S];
+    if (cl < nt) {
+      const long long c = c0 + cl;
+      double rn = rho - a.lambda * (fr - fl);
+      if (a.y0) rn = a.wa * r0 + a.wb * rn;
+      const double rinv = krs_rcp(rn);
+      if (a.rho_out) a.rho_out[c] = rn;
+      const bool lup = fl > 0.0, rup = fr > 0.0;
+#pragma unroll
+      for (int s = 0; s < S; ++s) {
+        const double yc = sy[(cl + 2) * LDY + s], dc = sd[(cl + 1) * LDY + s];
+        const double yl = lup ? sy[(cl + 1) * LDY + s] + sd[cl * LDY + s] : yc - dc;
+        const double yr = rup ? yc + dc : sy[(cl + 3) * LDY + s] - sd[(cl + 2) * LDY + s];
+        double un = rho * yc - a.lambda * (yr * fr - yl * fl);
+        if (a.y0) un = a.wa * r0 * a.y0[c * S + s] + a.wb * un;
+        out[s] = un * rinv;
+      }
+    }
+    __syncthreads();                                  // every thread has read sd
+    if (cl < nt) {
+#pragma unroll
+      for (int s = 0; s < S; ++s) sd[cl * LDY + s] = out[s];
+    }
+    __syncthreads();
+    double* dst = a.y_out + c0 * S;
+    if (LDY == S) { for (int i = tid; i < nt * S; i += T) dst[i] = sd[i]; }
+    else { for (int i = tid; i < nt * S; i += T) dst[i] = sd[(i / S) * LDY + (i % S)]; }
+  }
+}
+
+template <int S>
+inline cudaError_t kr_advect_cell_launch(const KrAdvectArgs& a, const double* P_host, cudaStream_t st) {
+  KrAdvectArgsP<S> ap;
+  ap.a = a;
+  for (int i = 0; i < S * S; ++i) ap.P[i] = P_host[i];
+  static int n_sm = 0;
+  if (n_sm == 0) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+  }
+  int per_sm = 0;
+  constexpr int T = KrAdvectTile<S>::T;
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kr_advect_cell_kernel<S>, T, 0);
+  const long long n_tiles = (a.n_cells + T - 1) / T;
+  const unsigned grid = unsigned(std::min<long long>(n_tiles, (long long)std::max(1, per_sm) * std::max(1, n_sm)));
+  kr_advect_cell_kernel<S><<<grid, T, 0, st>>>(ap);
+  return cudaGetLastError();
 }
