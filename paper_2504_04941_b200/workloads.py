@@ -558,3 +558,34 @@ def make_advection_batch(n_species: int, n_elem: int, n_cells: int, seed: int = 
     vel = np.sin(2 * np.pi * 2 * xi + 0.3) + 0.2
     flux = np.where(vel > 0, np.roll(rho, 1), rho) * vel
     return comp, np.ascontiguousarray(y), rho, flux
+
+
+# --------------------------------------------------------------------------
+# ray tracing (NEXT-3: PAPER.md section 3) -- inputs only, no method arithmetic
+# --------------------------------------------------------------------------
+
+def make_ray_case(shape=(16, 12, 10), n_oblique: int = 64, n_abs: int = 3, n_bins: int = 4, seed: int = BASE_SEED + 3000,
+                  spacing=(0.25, 0.25, 0.25), columns: bool = True):
+    """Seeded synthetic input of the Cartesian ray tracer: absorber densities with ten decades of optical depth per cell,
+    cross sections per absorber and energy bin, and rays -- one plane-parallel ray along +x through the centre of every
+    (y, z) column (the plane-parallel source of PAPER.md Fig. 2) plus n_oblique rays from points outside the mesh in
+    random directions (some miss the mesh).  Returns a dict of numpy arrays."""
+    rng = np.random.default_rng(seed)
+    nx, ny, nz = shape
+    h = np.asarray(spacing, np.float64)
+    n_dens = 10.0 ** rng.uniform(-3, 3, size=(n_abs, nx, ny, nz))
+    sigma = 10.0 ** rng.uniform(-2.5, 0.5, size=(n_abs, n_bins)) / (nx * h[0])        # tau per cell ~ 1e-7 .. 1e2
+    org, drc = [], []
+    if columns:
+        for j in range(ny):
+            for k in range(nz):
+                org.append([-1.0, (j + 0.5) * h[1], (k + 0.5) * h[2]]); drc.append([1.0, 0.0, 0.0])
+    centre = 0.5 * h * np.asarray(shape)
+    for _ in range(n_oblique):
+        d = rng.normal(size=3); d /= np.linalg.norm(d)
+        target = centre + rng.uniform(-0.7, 0.7, 3) * h * np.asarray(shape)           # some targets lie outside: misses
+        org.append(list(target - d * 2.0 * np.linalg.norm(h * np.asarray(shape)))); drc.append(list(d))
+    org = np.asarray(org, np.float64); drc = np.asarray(drc, np.float64)
+    L = 10.0 ** rng.uniform(0, 3, size=(org.shape[0], n_bins))
+    return dict(shape=tuple(shape), spacing=tuple(float(v) for v in h), origins=org, directions=drc, L=L, sigma=sigma,
+                n_dens=np.ascontiguousarray(n_dens))
