@@ -239,6 +239,24 @@ int kr_advect_species_1d(kr_recon *r, int64_t n_cells, const double *y, const do
                          double dt_over_dx, double dx, int32_t scheme, int32_t periodic, double wa, double wb,
                          const double *y0, const double *rho0, double *y_out, double *rho_out, void *cuda_stream);
 
+/* ---- Ray tracing on a uniform Cartesian mesh and the photo-reaction rates it feeds (section 3) ----
+ * Every ray is walked cell by cell (eqs. 23-24: the exit point is the smallest positive delta-l among the cell's surfaces); in each
+ * cell, for every energy bin k, tau_jk = sum_i n_i sigma_ik dl_j, every absorbing species i receives the rate coefficient
+ * L_jk sigma_ik dl_j / dV * (1 - exp(-tau_jk)) / tau_jk (eqs. 30-31) and the ray goes on with L_jk exp(-tau_jk) (eq. 29).  The
+ * result k_out[i] is the per-cell unary rate field the chemistry step takes as an aux row (KR_F_AUX_UNARY, eq. 17).
+ *   nx, ny, nz; spacing, lower: HOST [3] cell sizes and coordinates of the mesh's lower corner (lower NULL -> 0), cm
+ *   origins, directions [n_rays * 3] DEVICE (a ray that starts outside the mesh enters through the first face it meets; one that
+ *   misses leaves its photons untouched); L_in [n_rays * n_bins] DEVICE photons per second per ray and bin
+ *   sigma: HOST [n_abs * n_bins] cm^2; n_dens: DEVICE [n_abs * n_cells] cm^-3, cell = (ix * ny + iy) * nz + iz
+ *   k_out: DEVICE [n_abs * n_cells] s^-1, overwritten (zeroed, then accumulated over rays and bins: FP64 atomic adds, so cells
+ *   crossed by several rays are summed in an order that may differ between calls at rounding level)
+ *   L_out [n_rays * n_bins], path [n_rays] (total length inside the mesh): DEVICE, may be NULL.
+ * At most 8 absorbing species and 16 bins (KR_EUNSUPPORTED beyond).  Asynchronous on cuda_stream. */
+int kr_raytrace_cartesian(int32_t nx, int32_t ny, int32_t nz, const double *spacing, const double *lower, int64_t n_rays,
+                          const double *origins, const double *directions, int32_t n_bins, const double *L_in, int32_t n_abs,
+                          const double *sigma, const double *n_dens, double *k_out, double *L_out, double *path,
+                          void *cuda_stream);
+
 const char *kr_last_error(void);
 const char *kr_version(void);
 

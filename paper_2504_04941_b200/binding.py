@@ -27,7 +27,7 @@ EXPORTS = [
     "kr_network_get_options", "kr_set_stream", "kr_network_set_mapping", "kr_network_set_tuning", "kr_network_info",
     "kr_network_kernel_desc", "kr_network_spec_source", "kr_network_spec_compile", "kr_network_wpc_compile", "kr_network_row_compile", "kr_last_mixed_stats", "kr_thermochem_step", "kr_thermochem_step_ex", "kr_thermochem_step_host", "kr_last_launch_count",
     "kr_layout_cell_to_soa", "kr_layout_soa_to_cell", "kr_math_probe", "kr_measure_fp64_peak", "kr_last_error", "kr_version",
-    "kr_recon_create", "kr_recon_destroy", "kr_recon_projector", "kr_advect_species_1d",
+    "kr_recon_create", "kr_recon_destroy", "kr_recon_projector", "kr_advect_species_1d", "kr_raytrace_cartesian",
 ]
 
 _dp = C.POINTER(C.c_double)
@@ -116,6 +116,8 @@ def load() -> C.CDLL:
     lib.kr_recon_projector.argtypes = [vp, _dp, _ip]
     lib.kr_advect_species_1d.argtypes = [vp, C.c_int64, vp, vp, vp, C.c_double, C.c_double, C.c_int32, C.c_int32, C.c_double,
                                          C.c_double, vp, vp, vp, vp, vp]
+    lib.kr_raytrace_cartesian.argtypes = [C.c_int32, C.c_int32, C.c_int32, _dp, _dp, C.c_int64, vp, vp, C.c_int32, vp, C.c_int32,
+                                          _dp, vp, vp, vp, vp, vp]
     lib.kr_last_error.restype = C.c_char_p
     lib.kr_version.restype = C.c_char_p
     _lib = lib
@@ -375,3 +377,14 @@ class Recon:
         _check(load().kr_advect_species_1d(self._h, int(n_cells), _ptr(y), _ptr(rho), _ptr(mass_flux), float(dt_over_dx), float(dx),
                                            int(scheme), int(bool(periodic)), float(wa), float(wb), _ptr(y0), _ptr(rho0),
                                            _ptr(y_out), _ptr(rho_out), stream))
+
+
+def raytrace_cartesian(shape, spacing, n_rays, origins, directions, L_in, sigma, n_dens, k_out, L_out=None, path=None,
+                       lower=None, stream=None) -> None:
+    """kr_raytrace_cartesian: device tensors for the fields and rays, host arrays for spacing / lower / sigma."""
+    sp = _f64(np.asarray(spacing, np.float64)); lo = None if lower is None else _f64(np.asarray(lower, np.float64))
+    sg = _f64(np.asarray(sigma, np.float64))
+    n_abs, n_bins = int(sg.shape[0]), int(sg.shape[1])
+    _check(load().kr_raytrace_cartesian(int(shape[0]), int(shape[1]), int(shape[2]), _d(sp), _d(lo), int(n_rays), _ptr(origins),
+                                        _ptr(directions), n_bins, _ptr(L_in), n_abs, _d(sg), _ptr(n_dens), _ptr(k_out),
+                                        _ptr(L_out), _ptr(path), stream))
