@@ -24,6 +24,7 @@ struct KrHostNet {
   std::vector<unsigned> rstream[2];
   std::vector<int> rslot_ptr[2];
   int rlen[2] = {0, 0}, n_rslots[2] = {0, 0};
+  int row_compact = 0;           // 1: the row-layout term streams are in the compact two-factor form (see build_programs)
 };
 
 namespace kr_codegen {

@@ -301,6 +301,21 @@ __device__ __forceinline__ void entries(const KrNetDev& n, const Cell& c, const 
   const int* meta = n.emeta[W - 1] + G.gl;
   const int len = n.elen[W - 1];
   double acc = 0.0;
+#if KRR_COMPACT_TERMS
+  // compact form: {coef, byte offset of factor 0 | factor 1 << 16, destination entry (0xffff: none)}
+  (void)D; (void)meta;
+  const char* base = c.base;
+#pragma unroll 8
+  for (int i = 0; i < len; ++i) {
+    const uint4 t = __ldg(terms + i * GT);
+    const double coef = __hiloint2double((int)t.y, (int)t.x);
+    const double f0 = *reinterpret_cast<const double*>(base + (t.z & 0xffffu));
+    const double f1 = *reinterpret_cast<const double*>(base + (t.z >> 16));
+    acc = fma(coef * f0, f1, acc);
+    const unsigned dst = t.w & 0xffffu;
+    if (dst != 0xffffu) { J[dst] = acc; acc = 0.0; }
+  }
+#else
 #pragma unroll 4
   for (int i = 0; i < len; ++i) {
     const uint4 t = __ldg(terms + i * GT);
@@ -309,6 +324,7 @@ __device__ __forceinline__ void entries(const KrNetDev& n, const Cell& c, const 
     acc += coef * D[t.z & 0xffffu] * D[t.z >> 16] * D[t.w & 0xffffu] * D[t.w >> 16];
     if (dst >= 0) { J[dst] = acc; acc = 0.0; }
   }
+#endif
 }
 
 // ---- T row of J (eq. 20 with the dropped dC/dy term, DESIGN.md step 5): thread <-> column m; row S holds the raw heat sum
