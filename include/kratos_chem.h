@@ -169,6 +169,29 @@ int kr_thermochem_step_host(kr_network *net, int64_t n_cells, const double *rho,
                             int precision_mode, const double *aux, int32_t n_aux, int32_t *status,
                             kr_step_stats *stats);
 
+/* ---- Allocation-free variant of the step (callers that cannot call cudaMalloc: code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid it).  Same operation, same kernels and same results as kr_thermochem_step_ex in KR_FP64 for the
+ * networks the specialised thread-per-cell kernel serves (N <= 12 unknowns, default mapping: BASELINE configs 0, 1, 2;
+ * KR_EUNSUPPORTED otherwise, and when opts.retry != 0).  Its scratch -- 16 work / statistics counters and, for isothermal
+ * networks, the [2R + 1][n_cells] doubles the preliminary kernel hands to the solve kernel -- is a file-scope static device
+ * array of kr_static_scratch_bytes() = 16 MiB, which every GPU that loads the library holds until the process exits.
+ *   kr_static_setup(net)   once per device, with that device current, OUTSIDE any capture: resolves the device address of the
+ *                          array (cudaGetSymbolAddress) and runs the kernels once on zero cells; synchronises the handle's stream.
+ *   kr_static_max_cells    largest n_cells one call takes for this network: (16 MiB - 256 B) / (8 (2R + 1)) for isothermal
+ *                          networks (config 2, R = 9: 110 374 cells), INT64_MAX for networks with an energy equation.
+ *   kr_thermochem_step_static  arguments as kr_thermochem_step_ex (DEVICE pointers, in place, asynchronous on cuda_stream unless
+ *                          stats is non-NULL).  Calls no cudaMalloc, cudaFree or allocating library routine.  KR_EINVAL with a
+ *                          message naming the limit when n_cells needs more scratch than the array holds, or when
+ *                          kr_static_setup has not run on the current device.
+ * Every call on a device shares the one array, which keeps the last call's contents: the call clears the counters itself (the
+ * workspace is written before it is read), and two calls that overlap on the GPU (different streams, or different handles
+ * on the same device) RACE on it -- serialise them.  kr_last_mixed_stats and the retry procedure do not apply. */
+int64_t kr_static_scratch_bytes(void);
+int kr_static_setup(kr_network *net);
+int kr_static_max_cells(const kr_network *net, int64_t *max_cells);
+int kr_thermochem_step_static(kr_network *net, int64_t n_cells, const double *rho, double *T, double *y, double dt,
+                              const double *aux, int32_t n_aux, int32_t *status, kr_step_stats *stats, void *cuda_stream);
+
 /* One-line description of the kernel the current mapping launches (registers, blocks per SM ...), host buffer. */
 int kr_network_kernel_desc(const kr_network *net, char *buf, int64_t cap);
 /* The generated translation unit (struct KrNet of constexpr tables) the specialised kernel is compiled against;

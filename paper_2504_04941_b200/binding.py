@@ -28,6 +28,7 @@ EXPORTS = [
     "kr_network_kernel_desc", "kr_network_spec_source", "kr_network_spec_compile", "kr_network_wpc_compile", "kr_network_row_compile", "kr_last_mixed_stats", "kr_thermochem_step", "kr_thermochem_step_ex", "kr_thermochem_step_host", "kr_last_launch_count",
     "kr_layout_cell_to_soa", "kr_layout_soa_to_cell", "kr_math_probe", "kr_measure_fp64_peak", "kr_last_error", "kr_version",
     "kr_recon_create", "kr_recon_destroy", "kr_recon_projector", "kr_advect_species_1d", "kr_raytrace_cartesian",
+    "kr_static_scratch_bytes", "kr_static_setup", "kr_static_max_cells", "kr_thermochem_step_static",
 ]
 
 _dp = C.POINTER(C.c_double)
@@ -96,6 +97,12 @@ def load() -> C.CDLL:
                                           C.POINTER(StepStats), vp]
     lib.kr_thermochem_step_host.argtypes = [vp, C.c_int64, vp, vp, vp, C.c_double, C.c_int, vp, C.c_int32, vp,
                                             C.POINTER(StepStats)]
+    lib.kr_static_scratch_bytes.argtypes = []
+    lib.kr_static_scratch_bytes.restype = C.c_int64
+    lib.kr_static_setup.argtypes = [vp]
+    lib.kr_static_max_cells.argtypes = [vp, C.POINTER(C.c_int64)]
+    lib.kr_thermochem_step_static.argtypes = [vp, C.c_int64, vp, vp, vp, C.c_double, vp, C.c_int32, vp,
+                                              C.POINTER(StepStats), vp]
     lib.kr_last_launch_count.argtypes = [vp]
     lib.kr_network_kernel_desc.argtypes = [vp, C.c_char_p, C.c_int64]
     lib.kr_network_spec_source.argtypes = [C.POINTER(NetworkDesc), C.c_char_p, C.c_int64]
@@ -331,6 +338,29 @@ class Network:
                                               int(precision_mode), _ptr(aux), n_aux, _ptr(status),
                                               C.byref(st) if want_stats else None))
         return st.as_dict() if want_stats else None
+
+    # -- the allocation-free variant (static device scratch; include/kratos_chem.h) ---------------
+    def static_setup(self) -> None:
+        _check(load().kr_static_setup(self._h))
+
+    def static_max_cells(self) -> int:
+        m = C.c_int64()
+        _check(load().kr_static_max_cells(self._h, C.byref(m)))
+        return int(m.value)
+
+    def thermochem_step_static(self, n_cells: int, rho, T, y, dt: float, aux=None, status=None, want_stats: bool = False,
+                               stream: int = 0) -> Optional[dict]:
+        """kr_thermochem_step_static: as thermochem_step_ex in fp64, no allocation inside the call."""
+        n_aux = 0 if aux is None else int(aux.shape[0])
+        st = StepStats()
+        _check(load().kr_thermochem_step_static(self._h, int(n_cells), _ptr(rho), _ptr(T), _ptr(y), float(dt),
+                                                _ptr(aux), n_aux, _ptr(status), C.byref(st) if want_stats else None,
+                                                C.c_void_p(stream or None)))
+        return st.as_dict() if want_stats else None
+
+
+def static_scratch_bytes() -> int:
+    return int(load().kr_static_scratch_bytes())
 
 
 def math_probe(x, rcp, ex, n: int, stream: int = 0) -> None:
