@@ -15,9 +15,10 @@
 //                       pivot row, the lane that holds it writes its row to shared memory once, every lane reads it
 //                       back as a broadcast and applies the rank-1 update to its own row: N - k independent FMAs per
 //                       lane against (N - k) / 2 broadcast 16-byte loads, one warp-level sync per column, no shuffles,
-//                       no dynamic register indexing (the column loop is unrolled, rows never move: a used row is
-//                       marked, and the update is applied to used rows as well -- the Gauss-Jordan form -- so that after
-//                       N columns row p_k holds x_k * pivot_k and no substitution pass is needed).  The system that is
+//                       no dynamic register indexing (the column loop is rolled and the row shifts by one register per
+//                       column, see struct Elim; a used row is marked, and the update is applied to used rows as well --
+//                       the Gauss-Jordan form -- so that after N columns row p_k holds x_k * pivot_k in its first
+//                       register and no substitution pass is needed).  The system that is
 //                       eliminated is step 6's (I - hJ) delta = -G multiplied through by -1/h, (J - I/h) delta = G/h:
 //                       same pivots under implicit row scaling, same solution, and the rows of J load into registers
 //                       as they are.
@@ -59,7 +60,16 @@ constexpr int oDQT = oQ + 8 * R;                        // [R]  dq_r/dT (energy)
 constexpr int oQH = oDQT + (ENERGY ? 8 * R : 0);        // [R]  k_f P' - k_r P'' (third body)
 constexpr int oMT = oQH + (KRR_ANY_TB ? 8 * R : 0);     // [R]  M_r
 constexpr int oRED = oMT + (KRR_ANY_TB ? 8 * R : 0);    // [8 W + 4] reduction scratch, cell slot, scalars
-constexpr int oKEY = oRED + 8 * (8 * W + 4);            // int[2][W][2] pivot keys of the two warps (double buffered)
+constexpr int oPK = oRED + 8 * (8 * W + 4);             // [W][12] per-warp parking slots of the controller state + [6] counters
+constexpr int oKEY = oPK + 8 * (12 * W + 6);            // int[2][W][2] pivot keys of the two warps (double buffered)
+#ifndef KRR_RU
+#define KRR_RU 3
+#endif
+constexpr int RU = KRR_RU;                              // reactions in flight per thread (reactions())
+#ifndef KRR_SB
+#define KRR_SB 8
+#endif
+constexpr int SB = KRR_SB;                              // steps per batch of the term streams (the host pads to it)
 constexpr int NSLOT = KRR_NSLOT;                        // partial sums of the row program (host-built chunks)
 constexpr int oPART = a16(oKEY + 4 * 2 * W * 2);        // [NSLOT] partial f sums, then (energy) [NSLOT] partial T-column sums
 constexpr int oUR = a16(oPART + 8 * NSLOT * (ENERGY ? 2 : 1));   // [2][W][2 (NC2 + 1)] published pivot-row candidates + reciprocal (double buffered)
@@ -73,8 +83,14 @@ static_assert(!KRR_ANY_TB || (oQH == 8 * KRR_I_QH && oMT == 8 * KRR_I_MT), "host
 static_assert(LDJ == KRR_LDJ, "host and device disagree on the row stride of J");
 #endif
 
+// shared-memory accesses of the term streams by 32-bit shared-window address: the base is converted once per evaluation (the
+// compiler otherwise rebuilds it from a special register in front of every access with a data-dependent offset)
+__device__ __forceinline__ double lds(unsigned a) { double v; asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a)); return v; }
+__device__ __forceinline__ void sts(unsigned a, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v)); }
+
 struct Cell {
   char* base;
+  unsigned sb;                     // the same address in the shared window (set by eval)
   __device__ __forceinline__ double* d(int off) const { return reinterpret_cast<double*>(base + off); }
   __device__ __forceinline__ int* i(int off) const { return reinterpret_cast<int*>(base + off); }
   __device__ __forceinline__ double& F(int row) const { return d(oJ)[row * LDJ + N]; }
@@ -182,72 +198,119 @@ __device__ __forceinline__ void reactions(const KrNetDev& n, const Cell& c, cons
                                           bool computeK, double& heat_sum, double& heat_dT) {
   double *NN = c.d(oNN), *TH = c.d(oTH), *KF = c.d(oKF), *KR = c.d(oKR), *Q = c.d(oQ);
   heat_sum = 0.0; heat_dT = 0.0;
-  for (int r = G.gl; r < R; r += GT) {
-    // every table value of the reaction is requested up front: independent loads, one exposed latency instead of a chain
-    const int fl = __ldg(n.flags + r);
-    const int2* fp = reinterpret_cast<const int2*>(n.fac + 6 * r);
-    const int2 f01 = __ldg(fp), f23 = __ldg(fp + 1), f45 = __ldg(fp + 2);
-    const double A_r = __ldg(n.A + r);
-    const double qk = KRR_ANY_QEXT ? __ldg(n.qk + r) : 0.0;
-    double beta = 0.0, Ea = 0.0, c0 = 0.0;
-    int dn_tot = 0;
-    int4 tg0 = make_int4(0, 0, 0, 0), tg1 = make_int4(0, 0, 0, 0);
-    if (computeK) {
-      beta = __ldg(n.beta + r); Ea = __ldg(n.Ea + r); c0 = __ldg(n.c0 + r);
-      if (KRR_ANY_REV) {
-        dn_tot = __ldg(n.dnu_tot + r);
-        const int4* tp = reinterpret_cast<const int4*>(n.tgt + 8 * r);
-        tg0 = __ldg(tp); tg1 = __ldg(tp + 1);
-      }
+  // RU reactions per thread are in flight at a time, stage by stage and without branches on the kind of the reaction
+  // (the kinds are selected at the end of a stage): the exponentials and the table loads of different reactions are
+  // independent chains, and a thread that took them one reaction after the other waited for each in turn.
+  for (int r0 = G.gl; r0 < R; r0 += GT * RU) {
+    int fl[RU], rr[RU];
+    bool on[RU];
+    int2 f01[RU], f23[RU], f45[RU];
+    double A_r[RU], qk[RU], kf[RU], kr[RU], dlf[RU], dlr[RU];
+    // ---- stage 1: every table value of the reactions is requested up front ----
+#pragma unroll
+    for (int u = 0; u < RU; ++u) {
+      const int r = r0 + u * GT;
+      on[u] = r < R; rr[u] = on[u] ? r : (R - 1);
+      fl[u] = __ldg(n.flags + rr[u]);
+      const int2* fp = reinterpret_cast<const int2*>(n.fac + 6 * rr[u]);
+      f01[u] = __ldg(fp); f23[u] = __ldg(fp + 1); f45[u] = __ldg(fp + 2);
+      A_r[u] = __ldg(n.A + rr[u]);
+      qk[u] = KRR_ANY_QEXT ? __ldg(n.qk + rr[u]) : 0.0;
+      kr[u] = 0.0; dlf[u] = 0.0; dlr[u] = 0.0;
     }
-    double kf, kr = 0.0, dlf = 0.0, dlr = 0.0;
     if (computeK) {
-      if (fl & KR_DF_CONST) kf = A_r;
-      else if (fl & KR_DF_AUX) {
-        const int ai = n.auxi[r];
-        kf = A_r * (ai > 0 ? aux[(long long)ai * n_cells + cell] : aux0);
-      } else {
-        const double lnkf = c0 + beta * lnT - Ea * invT;
-        kf = krs_exp(lnkf);
-        dlf = (beta + Ea * invT) * invT;
-        if (KRR_ANY_REV && (fl & KR_DF_REV)) {
-          double sg = 0.0, su = 0.0;
-          const int tg[8] = {tg0.x, tg0.y, tg0.z, tg0.w, tg1.x, tg1.y, tg1.z, tg1.w};
+      double beta[RU], Ea[RU], c0[RU], auxv[RU];
+      int dn_tot[RU];
+      int4 tg0[RU], tg1[RU];
+#pragma unroll
+      for (int u = 0; u < RU; ++u) {
+        beta[u] = __ldg(n.beta + rr[u]); Ea[u] = __ldg(n.Ea + rr[u]); c0[u] = __ldg(n.c0 + rr[u]);
+        dn_tot[u] = 0; tg0[u] = make_int4(0, 0, 0, 0); tg1[u] = make_int4(0, 0, 0, 0);
+        if (KRR_ANY_REV) {
+          dn_tot[u] = __ldg(n.dnu_tot + rr[u]);
+          const int4* tp = reinterpret_cast<const int4*>(n.tgt + 8 * rr[u]);
+          tg0[u] = __ldg(tp); tg1[u] = __ldg(tp + 1);
+        }
+        auxv[u] = aux0;
+        if (KRR_NAUX > 0 && (fl[u] & KR_DF_AUX)) {
+          const int ai = n.auxi[rr[u]];
+          if (ai > 0) auxv[u] = aux[(long long)ai * n_cells + cell];
+        }
+      }
+      // ---- stage 2: Arrhenius form for every reaction (eq. 16 with R4), detailed balance (R5) where reversible ----
+      double lnkf[RU], kfa[RU];
+#pragma unroll
+      for (int u = 0; u < RU; ++u) lnkf[u] = c0[u] + beta[u] * lnT - Ea[u] * invT;
+#pragma unroll
+      for (int u = 0; u < RU; ++u) kfa[u] = krs_exp(lnkf[u]);
+      if (KRR_ANY_REV) {
+        double sg[RU], su[RU], kra[RU];
+#pragma unroll
+        for (int u = 0; u < RU; ++u) {
+          sg[u] = 0.0; su[u] = 0.0;
+          const int tg[8] = {tg0[u].x, tg0[u].y, tg0[u].z, tg0[u].w, tg1[u].x, tg1[u].y, tg1[u].z, tg1[u].w};
 #pragma unroll
           for (int t = 0; t < 7; ++t)
             if (t < tg[0]) {
               const int e = tg[1 + t];
               const double cf = (double)((e >> 8) - 128);
-              sg += cf * TH[e & 255];
-              su += cf * TH[S + (e & 255)];
+              sg[u] += cf * TH[e & 255];
+              su[u] += cf * TH[S + (e & 255)];
             }
-          const double lnKc = -sg + (double)dn_tot * (n.ln_p0_kB - lnT);
-          kr = krs_exp(lnkf - lnKc);
-          dlr = dlf - su * invT;
+        }
+#pragma unroll
+        for (int u = 0; u < RU; ++u) {
+          const double lnKc = -sg[u] + (double)dn_tot[u] * (n.ln_p0_kB - lnT);
+          kra[u] = krs_exp(lnkf[u] - lnKc);
+        }
+#pragma unroll
+        for (int u = 0; u < RU; ++u) {
+          const bool arr = !(fl[u] & (KR_DF_CONST | KR_DF_AUX)), rev = arr && (fl[u] & KR_DF_REV);
+          const double d = arr ? (beta[u] + Ea[u] * invT) * invT : 0.0;
+          kr[u] = rev ? kra[u] : 0.0;
+          dlr[u] = rev ? d - su[u] * invT : 0.0;
         }
       }
-      KF[r] = kf;
-      if (KRR_ANY_REV) KR[r] = kr;
+#pragma unroll
+      for (int u = 0; u < RU; ++u) {
+        const bool arr = !(fl[u] & (KR_DF_CONST | KR_DF_AUX));
+        dlf[u] = arr ? (beta[u] + Ea[u] * invT) * invT : 0.0;
+        kf[u] = (fl[u] & KR_DF_CONST) ? A_r[u] : ((fl[u] & KR_DF_AUX) ? A_r[u] * auxv[u] : kfa[u]);
+      }
     } else {
-      kf = KF[r];
-      if (KRR_ANY_REV) kr = KR[r];
+#pragma unroll
+      for (int u = 0; u < RU; ++u) {
+        kf[u] = KF[rr[u]];
+        if (KRR_ANY_REV) kr[u] = KR[rr[u]];
+      }
     }
-    const double Pf = NN[f01.x] * NN[f01.y] * NN[f23.x];
-    const double Pr = NN[f23.y] * NN[f45.x] * NN[f45.y];
-    double Mtb = 1.0;
-    const double qhat = kf * Pf - kr * Pr;
-    if (KRR_ANY_TB && (fl & KR_DF_TB)) {
-      Mtb = 0.0;
-      for (int s = 0; s < S; ++s) Mtb += n.tb_eff[r * S + s] * NN[s];
-      c.d(oQH)[r] = qhat; c.d(oMT)[r] = Mtb;
+    // ---- stage 3: mass-action products, q_r, dq_r/dT (loads of all reactions first, then the stores) ----
+    double Pf[RU], Pr[RU], Mtb[RU];
+#pragma unroll
+    for (int u = 0; u < RU; ++u) {
+      Pf[u] = NN[f01[u].x] * NN[f01[u].y] * NN[f23[u].x];
+      Pr[u] = NN[f23[u].y] * NN[f45[u].x] * NN[f45[u].y];
+      Mtb[u] = 1.0;
+      if (KRR_ANY_TB && (fl[u] & KR_DF_TB)) {
+        Mtb[u] = 0.0;
+        for (int s = 0; s < S; ++s) Mtb[u] += n.tb_eff[rr[u] * S + s] * NN[s];
+      }
     }
-    const double q = Mtb * qhat;
-    Q[r] = q;
-    heat_sum += qk * q;
-    if (ENERGY) {
-      const double dqdT = Mtb * (kf * dlf * Pf - kr * dlr * Pr);
-      c.d(oDQT)[r] = dqdT;
-      heat_dT += qk * dqdT;
+#pragma unroll
+    for (int u = 0; u < RU; ++u) {
+      if (!on[u]) continue;
+      const int r = rr[u];
+      if (computeK) { KF[r] = kf[u]; if (KRR_ANY_REV) KR[r] = kr[u]; }
+      const double qhat = kf[u] * Pf[u] - kr[u] * Pr[u];
+      if (KRR_ANY_TB && (fl[u] & KR_DF_TB)) { c.d(oQH)[r] = qhat; c.d(oMT)[r] = Mtb[u]; }
+      const double q = Mtb[u] * qhat;
+      Q[r] = q;
+      heat_sum += qk[u] * q;
+      if (ENERGY) {
+        const double dqdT = Mtb[u] * (kf[u] * dlf[u] * Pf[u] - kr[u] * dlr[u] * Pr[u]);
+        c.d(oDQT)[r] = dqdT;
+        heat_dT += qk[u] * dqdT;
+      }
     }
   }
 }
@@ -258,22 +321,44 @@ __device__ __forceinline__ void reactions(const KrNetDev& n, const Cell& c, cons
 // as ONE coalesced stream of 8-byte words.  Pass 2, thread <-> species: the few partial sums of a species, in chunk
 // order (a fixed order: results do not depend on which thread summed what).
 __device__ __forceinline__ void row_partials(const KrNetDev& n, const Cell& c, const Grp& G) {
-  const double *Q = c.d(oQ), *DQT = c.d(oDQT);
-  double* PART = c.d(oPART);
+  const unsigned sQ = c.sb + oQ, sD = c.sb + oDQT, sP = c.sb + oPART;
   const uint2* rs = n.rstream[W - 1] + G.gl;
-  const int len = n.rlen[W - 1];
+  const int nb = n.rlen[W - 1] / SB;           // batches of SB steps (the host pads to it)
+  // A batch requests all of its operands before its first sum, and the stream words of the next batch before that: the
+  // stores of the partial sums close a batch, not a step, and the latency of the stream (L2) hides under the batch in
+  // front of it.
   double af = 0.0, at = 0.0;
-#pragma unroll 4
-  for (int i = 0; i < len; ++i) {
-    const uint2 t = __ldg(rs + i * GT);
-    const int r = (int)(t.x & 0xffffu);
-    const double dnu = (double)((int)(t.x >> 16) - 128);
-    af += dnu * Q[r];
-    if (ENERGY) at += dnu * DQT[r];
-    if ((int)t.y >= 0) {
-      PART[t.y] = af; af = 0.0;
-      if (ENERGY) { PART[NSLOT + t.y] = at; at = 0.0; }
+  uint2 ta[SB], tb[SB];
+  auto load = [&](uint2 (&t)[SB], int b) {
+#pragma unroll
+    for (int q = 0; q < SB; ++q) t[q] = __ldg(rs + (b * SB + q) * GT);
+  };
+  auto work = [&](const uint2 (&t)[SB]) {
+    double qv[SB], dv[SB];
+#pragma unroll
+    for (int q = 0; q < SB; ++q) {
+      const unsigned r8 = (t[q].x & 0xffffu) * 8u;
+      qv[q] = lds(sQ + r8);
+      dv[q] = ENERGY ? lds(sD + r8) : 0.0;
     }
+#pragma unroll
+    for (int q = 0; q < SB; ++q) {
+      const double dnu = (double)((int)(t[q].x >> 16) - 128);
+      af = fma(dnu, qv[q], af);
+      if (ENERGY) at = fma(dnu, dv[q], at);
+      if ((int)t[q].y >= 0) {
+        sts(sP + 8u * t[q].y, af); af = 0.0;
+        if (ENERGY) { sts(sP + 8u * (NSLOT + t[q].y), at); at = 0.0; }
+      }
+    }
+  };
+  load(ta, 0);
+  for (int b = 0; b < nb; b += 2) {
+    if (b + 1 < nb) load(tb, b + 1);
+    work(ta);
+    if (b + 1 >= nb) break;
+    if (b + 2 < nb) load(ta, b + 2);
+    work(tb);
   }
 }
 __device__ __forceinline__ void row_combine(const KrNetDev& n, const Cell& c, const Grp& G, double invN, bool wantJ) {
@@ -294,35 +379,53 @@ __device__ __forceinline__ void row_combine(const KrNetDev& n, const Cell& c, co
 // group finish together.  No read-modify-write of shared memory, no atomics, fixed order (replaces PAPER.md:232).
 // Entries that are structurally zero are never written: J is zeroed once per block.
 __device__ __forceinline__ void entries(const KrNetDev& n, const Cell& c, const Grp& G) {
-  const double* D = c.d(0);
-  double* J = c.d(oJ);
-  // {coef lo, coef hi, g0 | g1 << 16, g2 | g3 << 16}: one coalesced 16-byte load per thread and step, no dependent loads
+  // {coef lo, coef hi, g0 | g1 << 16, g2 | g3 << 16}: one coalesced 16-byte load per thread and step, no dependent loads.
+  // Batches of SB steps as in row_partials.
   const uint4* terms = reinterpret_cast<const uint4*>(n.estream[W - 1]) + G.gl;
-  const int* meta = n.emeta[W - 1] + G.gl;
-  const int len = n.elen[W - 1];
+  const int nb = n.elen[W - 1] / SB;
+  const unsigned sb = c.sb, sJ = c.sb + oJ;
   double acc = 0.0;
 #if KRR_COMPACT_TERMS
   // compact form: {coef, byte offset of factor 0 | factor 1 << 16, destination entry (0xffff: none)}
-  (void)D; (void)meta;
-  const char* base = c.base;
-#pragma unroll 8
-  for (int i = 0; i < len; ++i) {
-    const uint4 t = __ldg(terms + i * GT);
-    const double coef = __hiloint2double((int)t.y, (int)t.x);
-    const double f0 = *reinterpret_cast<const double*>(base + (t.z & 0xffffu));
-    const double f1 = *reinterpret_cast<const double*>(base + (t.z >> 16));
-    acc = fma(coef * f0, f1, acc);
-    const unsigned dst = t.w & 0xffffu;
-    if (dst != 0xffffu) { J[dst] = acc; acc = 0.0; }
+  uint4 ta[SB], tb[SB];
+  auto load = [&](uint4 (&t)[SB], int b) {
+#pragma unroll
+    for (int q = 0; q < SB; ++q) t[q] = __ldg(terms + (b * SB + q) * GT);
+  };
+  auto work = [&](const uint4 (&t)[SB]) {
+    double p[SB], f1[SB];
+#pragma unroll
+    for (int q = 0; q < SB; ++q) {
+      p[q] = lds(sb + (t[q].z & 0xffffu));
+      f1[q] = lds(sb + (t[q].z >> 16));
+    }
+#pragma unroll
+    for (int q = 0; q < SB; ++q) p[q] *= __hiloint2double((int)t[q].y, (int)t[q].x);
+#pragma unroll
+    for (int q = 0; q < SB; ++q) {
+      acc = fma(p[q], f1[q], acc);
+      const unsigned dst = t[q].w & 0xffffu;
+      if (dst != 0xffffu) { sts(sJ + 8u * dst, acc); acc = 0.0; }
+    }
+  };
+  load(ta, 0);
+  for (int b = 0; b < nb; b += 2) {
+    if (b + 1 < nb) load(tb, b + 1);
+    work(ta);
+    if (b + 1 >= nb) break;
+    if (b + 2 < nb) load(ta, b + 2);
+    work(tb);
   }
 #else
+  const int* meta = n.emeta[W - 1] + G.gl;
+  const int len = nb * SB;
 #pragma unroll 4
   for (int i = 0; i < len; ++i) {
     const uint4 t = __ldg(terms + i * GT);
     const int dst = __ldg(meta + i * GT);
     const double coef = __hiloint2double((int)t.y, (int)t.x);
-    acc += coef * D[t.z & 0xffffu] * D[t.z >> 16] * D[t.w & 0xffffu] * D[t.w >> 16];
-    if (dst >= 0) { J[dst] = acc; acc = 0.0; }
+    acc += coef * lds(sb + 8u * (t.z & 0xffffu)) * lds(sb + 8u * (t.z >> 16)) * lds(sb + 8u * (t.w & 0xffffu)) * lds(sb + 8u * (t.w >> 16));
+    if (dst >= 0) { sts(sJ + 8u * dst, acc); acc = 0.0; }
   }
 #endif
 }
@@ -338,9 +441,14 @@ __device__ __forceinline__ void trow(const Cell& c, const Grp& G, double T, doub
 }
 
 // ---- full evaluation of f (and J) at U.  Thermo / KF / KR valid as the flags say.
-__device__ __forceinline__ void eval(const KrNetDev& n, const Cell& c, const Grp& G, double Ncal, double T, double aux0,
+__device__ __forceinline__ void eval(const KrNetDev& n, const Cell& c_in, const Grp& G, double Ncal, double T, double aux0,
                                   const double* __restrict__ aux, long long cell, long long n_cells, bool computeK,
                                   bool wantJ) {
+  Cell c = c_in;
+  {                                  // the shared-window address of the cell, opaque to the compiler: converted once per
+    const unsigned sb0 = (unsigned)__cvta_generic_to_shared(c_in.base);     // evaluation and held in a register while it runs
+    asm volatile("mov.u32 %0, %1;" : "=r"(c.sb) : "r"(sb0));
+  }
   const double invT = krs_rcp(T), lnT = (ENERGY || computeK) ? log(T) : 0.0;
   const double invN = krs_rcp(Ncal);
   double *U = c.d(oU), *TH = c.d(oTH), *NN = c.d(oNN), *J = c.d(oJ);
@@ -387,152 +495,189 @@ __device__ __forceinline__ void eval(const KrNetDev& n, const Cell& c, const Grp
 // word) names the pivot row: Algorithm 1's scaled pivot, candidates closer than 2^-46 relative counting as tied, ties to
 // the smallest row (reading R14' of DESIGN.md).  A used row carries a negative scale: its key is negative and loses
 // against every candidate.
-#ifndef KRR_KEY64
-#define KRR_KEY64 1      // 0: 32-bit keys, one REDUX (measured: +5 % throughput, but candidates within 2^-14 tie, and on config 4
-#endif                   // that changed the accept / reject path of cells whose decisions have wide margins) -- kept for experiments only
-#if KRR_KEY64
-// the whole bit pattern of |a| / scale with the row in the 6 low bits (ties to 2^-46), two REDUX
+// (32-bit keys -- one REDUX -- were measured at +5 % throughput, but candidates within 2^-14 then tie, and on config 4 that
+// changed the accept / reject path of cells whose decisions have wide margins: not built.)
 typedef long long Key;
 __device__ __forceinline__ Key key_of(double v, double sc, int row) {
   return (__double_as_longlong(fabs(v) * sc) | 63LL) - (long long)row;
 }
-__device__ __forceinline__ Key warp_max_key(Key k) {
-  const int hi = (int)(k >> 32);
-  const unsigned lo = (unsigned)k;
-  const int H = __reduce_max_sync(0xffffffffu, hi);
-  const unsigned L = __reduce_max_sync(0xffffffffu, (hi == H) ? lo : 0u);
-  return ((long long)H << 32) | (long long)L;
-}
-#else
-typedef int Key;
-__device__ __forceinline__ Key key_of(double v, double sc, int row) {
-  return (__double2hiint(fabs(v) * sc) | 63) - row;
-}
-__device__ __forceinline__ Key warp_max_key(Key k) { return __reduce_max_sync(0xffffffffu, k); }
-#endif
 
-// The elimination state of one thread; the column loop is a compile-time recursion (run<K>), so that every register
-// index is static whatever N is.
+// The elimination state of one thread.  The column loop is a ROLLED loop: on this chip a kernel whose hot path is more
+// than ~32 KB of straight-line code is bound by instruction fetch (measured with a microbenchmark: 1.5 instructions per
+// clock and SM with 8-12 warps at different places of 64 KB+ of code, against 3 when the code fits the instruction
+// caches), and an unrolled column loop is 60 KB (N = 33) to 140 KB (N = 64).  Register indices stay static because the
+// row SHIFTS: the update of column k writes entry j of the row into the register of entry j - 1, so that entry 0 is
+// always the column being eliminated and the right-hand side the last live entry, and the pivot row is published (and
+// read back) in the same shifted layout.  The row shrinks by one entry per column; the loop is cut into SEG segments,
+// each compiled for the width the row has at its start (entries beyond the right-hand side are dead: neither published
+// nor updated).
 //
-// The column loop is software-pipelined: as soon as the update of column k has produced the entries of column k + 1 the
-// search for pivot k + 1 is started (candidate keys, REDUX, a speculative reciprocal of every candidate), and the
-// remaining FMAs of update k are issued behind it, so that the latency of the search hides under the update.  The lane
-// that wins publishes its row together with its reciprocal.
+// The loop is software-pipelined: as soon as the update of column k has produced the entries of column k + 1 the search
+// for pivot k + 1 is started, and the two reductions of the search are issued BETWEEN the chunks of the remaining update
+// (a warp issues in order: a reduction that waits for the one in front of it would hold up everything behind it), with
+// the pivot-row reads of a chunk requested one chunk ahead.  The lane that wins publishes its row with its reciprocal.
 constexpr int XRD = XR > 0 ? XR : 1;
 constexpr int URS = NC2 + 1;                  // one published row: NC2 pairs + {reciprocal of its column-k entry, its key}
+#ifndef KRR_SEG
+#define KRR_SEG 8
+#endif
+constexpr int SEG = (N >= 4 * KRR_SEG) ? KRR_SEG : 1;
+constexpr int seg_lo(int i) { return (int)((long long)i * N / SEG); }
+#ifndef KRR_UCH
+#define KRR_UCH 6
+#endif
+constexpr int UCH = KRR_UCH;                  // pairs of the pivot row per chunk (two chunks in flight)
 
 struct Elim {
-  double2 a[NC2];                             // the lane's row of [J - I/h | G/h]
-  double xr[XRD][XQ];                         // spread rows: element j of spread row e in lane j % 32, slot j / 32
+  double2 a[NC2];                             // the lane's row of [J - I/h | G/h], shifted: a[0].x is the entry of the current column
+  double xr[XRD][XQ];                         // spread rows (not shifted): element j of spread row e in lane j % 32, slot j / 32
   double sc, xsc[XRD];                        // > 0: 1 / scale of a candidate row; < 0: used (or no row)
   double xk[XRD];                             // the spread rows' entries of the column being searched
   double myrp, xrp[XRD];                      // reciprocal pivot of the column in which the row was the pivot row ...
   int mycol, xcol[XRD];                       // ... and that column
   Key kw;                                     // the warp's best key for the column being searched
+  int khi, kH;                                // search in flight: high word of this lane's key, the warp's largest high word
+  unsigned klo;
   double rk;                                  // speculative reciprocal of this lane's candidate
   int gl, lane, wq;
   double2* URb;
   const Grp* G;
 
-  __device__ __forceinline__ double col(int k) const { return (k & 1) ? a[k >> 1].y : a[k >> 1].x; }
-
-  // candidate search for column KK on the rows as they stand: the warp's best key (REDUX), and the speculative
-  // reciprocal of this lane's candidate (overlaps the reduction; only the winner's is used)
-  template <int KK>
-  __device__ __forceinline__ void pick() {
-    const double ak = col(KK);
+  // candidate search for column kk on the rows as they stand (entry 0 of the shifted row), first half: this lane's key, the
+  // warp-wide maximum of the high words (REDUX), and the speculative reciprocal of this lane's candidate (only the
+  // winner's is used)
+  __device__ __forceinline__ void pick_a(int kk) {
+    const double ak = a[0].x;
     Key key = key_of(ak, sc, gl);
 #pragma unroll
-    for (int e = 0; e < XR; ++e) {             // element KK of a spread row sits in lane KK % 32: every lane gets it
-      xk[e] = __shfl_sync(0xffffffffu, xr[e][KK >> 5], KK & 31);
-      const Key kx = key_of(xk[e], xsc[e], NR + e);
-      key = (kx > key) ? kx : key;
+    for (int e = 0; e < XR; ++e) {             // element kk of a spread row sits in lane kk % 32, which enters it in the
+      double v = xr[e][0];                     // search beside its own row (no shuffle in front of the reduction); every
+#pragma unroll                                 // lane gets the value for the multiplier of the next update
+      for (int q = 1; q < XQ; ++q) v = ((kk >> 5) == q) ? xr[e][q] : v;
+      const Key kx = key_of(v, xsc[e], NR + e);
+      key = (lane == (kk & 31) && kx > key) ? kx : key;
+      xk[e] = __shfl_sync(0xffffffffu, v, kk & 31);
     }
-    kw = warp_max_key(key);
+    khi = (int)(key >> 32); klo = (unsigned)key;
+    kH = __reduce_max_sync(0xffffffffu, khi);
     rk = krs_rcp(ak);
   }
-  // publication of the warp's winner: its row from column KK on (every earlier update applied), the reciprocal of its
-  // column-KK entry and the key
-  template <int KK>
-  __device__ __forceinline__ void publish() {
-    constexpr int buf = KK & 1;
+  // second half: the maximum of the low words among the rows that share the largest high word
+  __device__ __forceinline__ void pick_b() {
+    const unsigned L = __reduce_max_sync(0xffffffffu, (khi == kH) ? klo : 0u);
+    kw = ((long long)kH << 32) | (long long)L;
+  }
+  // publication of the warp's winner for column kk: its row (WD entries from the current column on, every earlier update
+  // applied), the reciprocal of its current-column entry and the key
+  template <int WD>
+  __device__ __forceinline__ void publish(int kk) {
     const int pw = (kw >= 0) ? (63 - (int)(kw & 63)) : -1;
-    double2* URw = URb + (buf * W + wq) * URS;
+    double2* URw = URb + ((kk & 1) * W + wq) * URS;
     if (gl == pw) {
 #pragma unroll
-      for (int j = KK >> 1; j < NC2; ++j) URw[j] = a[j];
+      for (int j = 0; j < (WD + 1) / 2; ++j) URw[j] = a[j];
       URw[NC2] = make_double2(rk, __longlong_as_double((long long)kw));
     }
 #pragma unroll
     for (int e = 0; e < XR; ++e)
       if (pw == NR + e) {
 #pragma unroll
-        for (int q = 0; q < XQ; ++q)
-          if (lane + 32 * q < NC) reinterpret_cast<double*>(URw)[lane + 32 * q] = xr[e][q];
+        for (int q = 0; q < XQ; ++q) {
+          const int c = lane + 32 * q;         // absolute column; published at its distance from the current column
+          if (c >= kk && c < NC) reinterpret_cast<double*>(URw)[c - kk] = xr[e][q];
+        }
         if (lane == 0) URw[NC2] = make_double2(krs_rcp(xk[e]), __longlong_as_double((long long)kw));
       }
     if (W > 1 && pw < 0 && lane == 0) URw[NC2] = make_double2(0.0, __longlong_as_double(-1LL));   // no candidate in this warp
   }
 
-  template <int K>
-  __device__ __forceinline__ void column() {
-    constexpr int buf = K & 1, K2 = K >> 1;
-    // ---- the pivot row of column K: the warp's candidate, or the better of the two warps' candidates -------------------
+  // update of the pairs j0 .. j0 + UCH - 1 of the shifted row from the chunk u: entries 2j, 2j + 1 -> 2j - 1, 2j
+  template <int WD>
+  __device__ __forceinline__ void apply(int j0, double l, const double2 (&u)[UCH]) {
+    constexpr int NP = (WD + 1) / 2;
+#pragma unroll
+    for (int q = 0; q < UCH; ++q) {
+      const int j = j0 + q;
+      if (j < NP) {
+        a[j - 1].y = fma(l, u[q].x, a[j].x);
+        if (2 * j + 1 < WD) a[j].x = fma(l, u[q].y, a[j].y);
+      }
+    }
+  }
+  template <int WD>
+  __device__ __forceinline__ void fetch(int j0, const double2* URw, double2 (&u)[UCH]) {
+    constexpr int NP = (WD + 1) / 2;
+#pragma unroll
+    for (int q = 0; q < UCH; ++q)
+      if (j0 + q < NP) u[q] = URw[j0 + q];
+  }
+
+  // column k of a segment whose rows have WD live entries at its start (entry 0: column k, ..., the right-hand side last)
+  template <int WD>
+  __device__ __forceinline__ void column(int k) {
+    constexpr int NP = (WD + 1) / 2;                         // pairs of the row; pair 0 holds the current column
+    // ---- the pivot row of column k: the warp's candidate, or the better of the two warps' candidates -------------------
     Key kbest = kw;
-    const double2* URw = URb + (buf * W + wq) * URS;
+    const double2* URw = URb + ((k & 1) * W + wq) * URS;
     double2 tail;
     if (W > 1) {
       G->sync();
-      const double2 t0 = URb[(buf * W + 0) * URS + NC2], t1 = URb[(buf * W + 1) * URS + NC2];
+      const double2 t0 = URb[((k & 1) * W + 0) * URS + NC2], t1 = URb[((k & 1) * W + 1) * URS + NC2];
       const Key k0 = (Key)__double_as_longlong(t0.y), k1 = (Key)__double_as_longlong(t1.y);
       const bool second = k1 > k0;                           // keys carry the row: they are never equal unless both are -1
       kbest = second ? k1 : k0;
       tail = second ? t1 : t0;
-      URw = URb + (buf * W + (second ? 1 : 0)) * URS;
+      URw = URb + ((k & 1) * W + (second ? 1 : 0)) * URS;
     } else {
       __syncwarp();
       tail = URw[NC2];
     }
+    // ---- broadcast reads of the pivot row: pair 0 and the first chunk at once, every further chunk one chunk ahead ------
+    const double2 u0 = URw[0];
+    double2 ua[UCH], ub[UCH];
+    fetch<WD>(1, URw, ua);
     const int p = (kbest >= 0) ? (63 - (int)(kbest & 63)) : -1;
-    // ---- broadcast read of the pivot row and its reciprocal, rank-1 update of the lane's row -----------------------------
     const double rp = tail.x;
     const bool mine = (gl == p);
-    const double l = mine ? 0.0 : -(col(K) * rp);          // the pivot row itself is not updated
-    if (mine) { sc = -1.0; mycol = K; myrp = rp; }
+    const double l = mine ? 0.0 : -(a[0].x * rp);            // the pivot row itself is not updated
+    if (mine) { sc = -1.0; mycol = k; myrp = rp; }
     double xl[XRD];
 #pragma unroll
     for (int e = 0; e < XR; ++e) {
       const bool xmine = (p == NR + e);
       xl[e] = xmine ? 0.0 : -(xk[e] * rp);
-      if (xmine) { xsc[e] = -1.0; xcol[e] = K; xrp[e] = rp; }
+      if (xmine) { xsc[e] = -1.0; xcol[e] = k; xrp[e] = rp; }
     }
-    // column K + 1 first: its entries feed the next search
-    constexpr int J1 = (K & 1) ? K2 + 1 : K2;              // the pair that holds column K + 1
-    const double2 u1 = URw[J1];
-    if (K & 1) a[J1].x = fma(l, u1.x, a[J1].x);
-    else a[J1].y = fma(l, u1.y, a[J1].y);
+    // column k + 1 first: its entries feed the next search
+    a[0].x = fma(l, u0.y, a[0].y);
 #pragma unroll
     for (int e = 0; e < XR; ++e)
 #pragma unroll
       for (int q = 0; q < XQ; ++q) {
-        const int j = lane + 32 * q;
-        if (j > K && j < NC) xr[e][q] = fma(xl[e], reinterpret_cast<const double*>(URw)[j], xr[e][q]);
+        const int c = lane + 32 * q;
+        if (c > k && c < NC) xr[e][q] = fma(xl[e], reinterpret_cast<const double*>(URw)[c - k], xr[e][q]);
       }
-    // the search for pivot K + 1 is issued in front of the rest of update K; its winner publishes its row behind it
-    if constexpr (K + 1 < N) pick<K + 1>();
-    if (K & 1) a[J1].y = fma(l, u1.y, a[J1].y);
+    // the search for pivot k + 1 is issued in front of the rest of update k, its second reduction behind the first chunk
+    const bool more = k + 1 < N;
+    if (more) pick_a(k + 1);
+    if (NP <= 1 && more) pick_b();
 #pragma unroll
-    for (int j = J1 + 1; j < NC2; ++j) {
-      const double2 u = URw[j];
-      a[j].x = fma(l, u.x, a[j].x); a[j].y = fma(l, u.y, a[j].y);
+    for (int j0 = 1; j0 < NP; j0 += 2 * UCH) {
+      fetch<WD>(j0 + UCH, URw, ub);
+      apply<WD>(j0, l, ua);
+      if (j0 == 1 && more) pick_b();
+      fetch<WD>(j0 + 2 * UCH, URw, ua);
+      apply<WD>(j0 + UCH, l, ub);
     }
-    if constexpr (K + 1 < N) publish<K + 1>();
+    if (more) publish<WD - 1>(k + 1);
   }
 
-  template <int K>
-  __device__ __forceinline__ void run() {
-    column<K>();
-    if constexpr (K + 1 < N) run<K + 1>();
+  template <int SI>
+  __device__ __forceinline__ void segment() {
+    constexpr int k0 = seg_lo(SI), k1 = seg_lo(SI + 1);
+#pragma unroll 1
+    for (int k = k0; k < k1; ++k) column<NC - k0>(k);
+    if constexpr (SI + 1 < SEG) segment<SI + 1>();
   }
 };
 
@@ -592,13 +737,14 @@ __device__ __forceinline__ bool eliminate(const Cell& c, const Grp& G, double h)
   if (!rows_ok) return false;
 
   E.URb = reinterpret_cast<double2*>(c.d(oUR));
-  E.mycol = -1; E.myrp = 0.0; E.kw = -1; E.rk = 0.0;
+  E.mycol = -1; E.myrp = 0.0; E.kw = -1; E.rk = 0.0; E.khi = 0; E.kH = 0; E.klo = 0u;
 #pragma unroll
   for (int e = 0; e < XRD; ++e) { E.xcol[e] = -1; E.xrp[e] = 0.0; E.xk[e] = 0.0; if (e >= XR) E.xsc[e] = -1.0; }
 
-  E.template pick<0>();
-  E.template publish<0>();
-  E.template run<0>();
+  E.pick_a(0);
+  E.pick_b();
+  E.template publish<NC>(0);
+  E.template segment<0>();
 
   // every row must have been a pivot row, with |pivot| >= 1e-300 in the units of I - hJ (|pivot'| >= 1e-300 / h here) and finite
   const double rmax = 1e300 * h;
@@ -608,7 +754,7 @@ __device__ __forceinline__ bool eliminate(const Cell& c, const Grp& G, double h)
   ok = G.all(ok);
   if (!ok) return false;
   // row p_k now holds x_k * pivot_k in its right-hand-side slot
-  if (rin) X[E.mycol] = E.col(N) * E.myrp;
+  if (rin) X[E.mycol] = E.a[0].x * E.myrp;         // N shifts have brought the right-hand side to entry 0
 #pragma unroll
   for (int e = 0; e < XR; ++e)
     if (lane == (N & 31)) X[E.xcol[e]] = E.xr[e][N >> 5] * E.xrp[e];
@@ -627,6 +773,7 @@ kr_row_kernel(const KrNetDev n, const KrOptsDev o, const KrStepArgs a) {
   Cell c;
   G.g = 0; G.gl = threadIdx.x;                // one cell per block: every shared-memory offset is a compile-time constant
   c.base = kr_sm_raw;
+  c.sb = 0;
   G.red = c.d(oRED);
   volatile long long* cellslot = (volatile long long*)(c.d(oRED) + 8 * W);
   double *U = c.d(oU), *UN = c.d(oUN), *X = c.d(oX);
@@ -634,7 +781,12 @@ kr_row_kernel(const KrNetDev n, const KrOptsDev o, const KrStepArgs a) {
   for (int i = G.gl; i < N * LDJ; i += GT) c.d(oJ)[i] = 0.0;    // structural zeros of J: written once, never touched again
   G.sync();
 
-  unsigned long long c_acc = 0, c_rej = 0, c_newton = 0, c_rate = 0, c_failed = 0;   // thread 0 of the group
+  // The solver's counters (thread 0) and, across every elimination, the controller state of the cell live in shared
+  // memory: the elimination needs the register file for the row and for two chunks of the pivot row in flight.
+  volatile unsigned long long* CNT = reinterpret_cast<volatile unsigned long long*>(c.d(oPK) + 12 * W);   // acc rej newton rate failed
+  volatile double* PK = c.d(oPK) + 12 * (G.gl >> 5);
+  if (G.gl == 0)
+    for (int i = 0; i < 6; ++i) CNT[i] = 0ull;
 
   for (;;) {
     if (G.gl == 0) {
@@ -643,7 +795,7 @@ kr_row_kernel(const KrNetDev n, const KrOptsDev o, const KrStepArgs a) {
       *cellslot = idx;
     }
     G.sync();
-    const long long cell = *cellslot;
+    long long cell = *cellslot;
     G.sync();
     if (cell >= a.n_cells) break;
 
@@ -652,9 +804,9 @@ kr_row_kernel(const KrNetDev n, const KrOptsDev o, const KrStepArgs a) {
     double Tc = a.T[cell];
     if (Tc < n.T_lo) { Tc = n.T_lo; st |= KR_DST_T_CLAMPED; }
     if (Tc > n.T_hi) { Tc = n.T_hi; st |= KR_DST_T_CLAMPED; }
-    const double Ncal = a.rho[cell] * (1.0 / KR_M_U);
-    const double T_iso = Tc;
-    const double aux0 = (KRR_NAUX > 0) ? a.aux[cell] : 0.0;
+    double Ncal = a.rho[cell] * (1.0 / KR_M_U);
+    double T_iso = Tc;
+    double aux0 = (KRR_NAUX > 0) ? a.aux[cell] : 0.0;
     for (int s = G.gl; s < S; s += GT) { const double x = a.y[cell * S + s]; UN[s] = x; U[s] = x; }
     if (ENERGY && G.gl == 0) { UN[S] = Tc; U[S] = Tc; }
     G.sync();
@@ -682,7 +834,7 @@ kr_row_kernel(const KrNetDev n, const KrOptsDev o, const KrStepArgs a) {
       for (int k = 1; k <= K; ++k) {
         const double T = ENERGY ? U[S] : T_iso;
         if (ENERGY || (prelim && KRR_ANY_REV)) { thermo(n, c, G, T, krs_rcp(T), log(T)); G.sync(); }
-        if ((ENERGY || prelim) && !a.cost_out) c_rate++;
+        if ((ENERGY || prelim) && !a.cost_out && G.gl == 0) CNT[3] = CNT[3] + 1ull;
         eval(n, c, G, Ncal, T, aux0, a.aux, cell, a.n_cells, ENERGY || prelim, !prelim);
         if (prelim) {
           if (o.h0_mode == 1 || a.cost_out) {
@@ -705,8 +857,18 @@ kr_row_kernel(const KrNetDev n, const KrOptsDev o, const KrStepArgs a) {
           prelim = false; was_prelim = true;
           break;
         }
-        c_newton++;
-        if (!eliminate(c, G, h)) { ran = false; break; }
+        if (G.gl == 0) CNT[2] = CNT[2] + 1ull;
+        // park the controller state (every lane of a warp writes the same values to the warp's slots and reads them back)
+        PK[0] = t; PK[1] = h_floor; PK[2] = e_prev; PK[3] = Ncal; PK[4] = T_iso; PK[5] = aux0;
+        PK[6] = __longlong_as_double(cell);
+        PK[7] = __hiloint2double(st, n_acc); PK[8] = __hiloint2double(n_rej, it); PK[9] = __hiloint2double(k, last ? 1 : 0);
+        const bool solved = eliminate(c, G, h);
+        t = PK[0]; h_floor = PK[1]; e_prev = PK[2]; Ncal = PK[3]; T_iso = PK[4]; aux0 = PK[5];
+        cell = __double_as_longlong(PK[6]);
+        { const double w7 = PK[7], w8 = PK[8], w9 = PK[9];
+          st = __double2hiint(w7); n_acc = __double2loint(w7); n_rej = __double2hiint(w8); it = __double2loint(w8);
+          k = __double2hiint(w9); last = __double2loint(w9) != 0; }
+        if (!solved) { ran = false; break; }
         bool fin = true;
         double en = 0.0;
         for (int i = G.gl; i < N; i += GT) {
@@ -773,10 +935,10 @@ kr_row_kernel(const KrNetDev n, const KrOptsDev o, const KrStepArgs a) {
       G.sync();
       continue;
     }
-    c_acc += n_acc; c_rej += n_rej;
+    if (G.gl == 0) { CNT[0] = CNT[0] + (unsigned long long)n_acc; CNT[1] = CNT[1] + (unsigned long long)n_rej; }
     if (failed) {                                                 // R13: revert (the caller's buffers were never written)
       if (a.fail_list) { if (G.gl == 0) a.fail_list[atomicAdd(a.fail_count, 1ull)] = cell; }   // second attempt
-      else { c_failed++; if (a.status && G.gl == 0) a.status[cell] = st | KR_DST_FAILED; }
+      else if (G.gl == 0) { CNT[4] = CNT[4] + 1ull; if (a.status) a.status[cell] = st | KR_DST_FAILED; }
       G.sync();
       continue;
     }
@@ -793,7 +955,7 @@ kr_row_kernel(const KrNetDev n, const KrOptsDev o, const KrStepArgs a) {
     G.sync();
   }
   if (G.gl == 0) {
-    atomicAdd(a.stats + 0, c_acc); atomicAdd(a.stats + 1, c_rej); atomicAdd(a.stats + 2, c_newton);
-    atomicAdd(a.stats + 3, c_newton); atomicAdd(a.stats + 4, c_rate); atomicAdd(a.stats + 5, c_failed);
+    atomicAdd(a.stats + 0, CNT[0]); atomicAdd(a.stats + 1, CNT[1]); atomicAdd(a.stats + 2, CNT[2]);
+    atomicAdd(a.stats + 3, CNT[2]); atomicAdd(a.stats + 4, CNT[3]); atomicAdd(a.stats + 5, CNT[4]);
   }
 }
