@@ -17,6 +17,7 @@ numpy only.  Importing this module never loads the CUDA library.
 from __future__ import annotations
 
 import itertools
+import math
 from dataclasses import dataclass, field
 from typing import Dict, List, Optional, Tuple
 
@@ -589,3 +590,47 @@ def make_ray_case(shape=(16, 12, 10), n_oblique: int = 64, n_abs: int = 3, n_bin
     L = 10.0 ** rng.uniform(0, 3, size=(org.shape[0], n_bins))
     return dict(shape=tuple(shape), spacing=tuple(float(v) for v in h), origins=org, directions=drc, L=L, sigma=sigma,
                 n_dens=np.ascontiguousarray(n_dens))
+
+
+# --------------------------------------------------------------------------
+# tabulated reaction rates (NEXT-4: PAPER.md:171) -- inputs only: a table is DATA the user reads in; here it is filled from
+# the network's own rate law so that tests can compare the tabulated run with the analytic one
+# --------------------------------------------------------------------------
+
+@dataclass
+class RateTable:
+    ln_k: np.ndarray             # [n_tab, n_rho, n_T] natural log of the rate coefficient at the nodes
+    ln_rho0: float
+    d_ln_rho: float
+    ln_T0: float
+    d_ln_T: float
+    reactions: List[int]         # the reaction of the network each table replaces
+
+
+def make_rate_table(net: Network, reactions, T_range=(5.0e3, 3.0e5), n_T: int = 257, rho_range=(1.0e-24, 1.0e-14),
+                    n_rho: int = 1, rho_exponent: float = 0.0) -> RateTable:
+    """Tables of the listed (irreversible Arrhenius) reactions of ``net`` on nodes uniform in ln rho and ln T:
+    ln k = ln A + beta ln(T / T_REF) - Ea / T + rho_exponent ln(rho / rho_range[0]) (the density factor only makes the
+    table two-dimensional; 0 = none)."""
+    lnT = np.linspace(math.log(T_range[0]), math.log(T_range[1]), n_T)
+    lnr = np.linspace(math.log(rho_range[0]), math.log(rho_range[1]), n_rho) if n_rho > 1 else np.array([math.log(rho_range[0])])
+    ln_k = np.empty((len(reactions), n_rho, n_T))
+    for t, r in enumerate(reactions):
+        base = math.log(net.A[r]) + net.beta[r] * (lnT - math.log(T_REF)) - net.Ea_over_k[r] / np.exp(lnT)
+        ln_k[t] = base[None, :] + rho_exponent * (lnr[:, None] - lnr[0])
+    return RateTable(ln_k, float(lnr[0]), float(lnr[1] - lnr[0]) if n_rho > 1 else 1.0, float(lnT[0]),
+                     float(lnT[1] - lnT[0]) if n_T > 1 else 1.0, [int(r) for r in reactions])
+
+
+def tabulated_network(net: Network, table: RateTable) -> Network:
+    """``net`` with every tabulated reaction turned into an aux-scaled one (KR_F_AUX_UNARY, A = 1): its rate coefficient is
+    then the aux row n_aux + t of the cell, which the table interpolation fills."""
+    import copy
+    out = copy.deepcopy(net)
+    for t, r in enumerate(table.reactions):
+        assert net.flags[r] == 0, "only plain irreversible Arrhenius reactions are tabulated here"
+        out.flags[r] = F_AUX_UNARY
+        out.aux_index[r] = net.n_aux + t
+        out.A[r] = 1.0; out.beta[r] = 0.0; out.Ea_over_k[r] = 0.0
+    out.n_aux = net.n_aux + len(table.reactions)
+    return out
