@@ -364,6 +364,44 @@ def bench_advection(args, ctx) -> dict:
             "note": "the step before the chemistry step in the paper's cycle (PAPER.md section 2.1); input larger than L2 and L2 flushed between launches"}
 
 
+def bench_table_rates(args, ctx) -> dict:
+    """kr_table_rates for config 2's six thermal rate laws read from tables (n_rho = 1,
+    4 097 temperature nodes: 197 KB of table, resident in L2), on 2^24 cells with config 2's temperature and density
+    distributions.  Algorithmic bytes: 16 in (rho, T) + 8 per table out = 64 per cell."""
+    import torch
+    from paper_2504_04941_b200 import binding as B
+    dev = ctx["dev"]
+    n = args.advect_cells
+    net, cells, _ = w.make_config(2, 1 << 16)
+    table = w.make_rate_table(net, [0, 1, 3, 4, 6, 7], T_range=(50.0, 2.0e5), n_T=4097)
+    reps = (n + cells.n_cells - 1) // cells.n_cells
+    rho = torch.tensor(cells.rho, device=dev).repeat(reps)[:n].contiguous()
+    T = torch.tensor(cells.T, device=dev).repeat(reps)[:n].contiguous()
+    lnk = torch.tensor(table.ln_k, device=dev)
+    n_tab = int(lnk.shape[0])
+    out = torch.empty((n_tab, n), dtype=torch.float64, device=dev)
+    stream = torch.cuda.current_stream()
+    run = lambda: B.table_rates(lnk, table.ln_rho0, table.d_ln_rho, table.ln_T0, table.d_ln_T, rho, T, out, stream=stream.cuda_stream)
+    for _ in range(3):
+        run()
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for a, b in ev:
+        ctx["flush"].zero_()
+        a.record(stream); run(); b.record(stream)
+    torch.cuda.synchronize()
+    ms = float(np.mean([a.elapsed_time(b) for a, b in ev]))
+    bytes_launch = float(n) * (16 + 8 * n_tab)
+    peak, src = hbm_peak()
+    gbs = bytes_launch / (ms * 1e-3) / 1e9
+    return {"workload": f"table_rates_{n_tab}x4097", "dtype": "f64", "cells": n, "value": n / (ms * 1e-3), "unit": "cells/s",
+            "ms_per_launch": ms, "gpu_launches": args.steps,
+            "roofline": {"bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak, "traffic": None,
+                         "traffic_note": TRAFFIC_NOTE, "peak_source": src, "bytes_per_launch": bytes_launch},
+            "note": "tabulated reaction rates at the start of the chemistry step (PAPER.md:171); two log(), six exp() and two divides "
+                    "in FP64 per cell beside 64 B of traffic; input larger than L2 and L2 flushed between launches"}
+
+
 def worker(args, rank: int, local_rank: int, world: int) -> None:
     import torch
     import torch.distributed as dist
@@ -382,7 +420,7 @@ def worker(args, rank: int, local_rank: int, world: int) -> None:
                peak_tf=B.measure_fp64_peak(8192))
     if args.advection_only:
         if rank == 0:
-            print(json.dumps({"next": {"advection": bench_advection(args, ctx)}}), flush=True)
+            print(json.dumps({"next": {"advection": bench_advection(args, ctx), "table_rates": bench_table_rates(args, ctx)}}), flush=True)
         return
     if args.config is not None:
         runs = [(args.config, args.mode)]
@@ -397,6 +435,7 @@ def worker(args, rank: int, local_rank: int, world: int) -> None:
     advection = None
     if rank == 0 and world == 1 and args.config is None and not args.no_advection:
         advection = bench_advection(args, ctx)
+        table_rates = bench_table_rates(args, ctx)
     if rank == 0:
         head = next((r for r, (i, m) in zip(results, runs) if i == HEADLINE and m == "fp64"), results[0])
         line = dict(head)
@@ -413,7 +452,7 @@ def worker(args, rank: int, local_rank: int, world: int) -> None:
                                 "notes": r["config"]["notes"]} for r in results]
             line["gpu_launches"] = int(sum(r["gpu_launches"] for r in results))
         if advection is not None:
-            line["next"] = {"advection": advection}
+            line["next"] = {"advection": advection, "table_rates": table_rates}
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

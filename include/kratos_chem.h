@@ -280,6 +280,23 @@ int kr_raytrace_cartesian(int32_t nx, int32_t ny, int32_t nz, const double *spac
                           const double *sigma, const double *n_dens, double *k_out, double *L_out, double *path,
                           void *cuda_stream);
 
+/* ---- Tabulated reaction rates (rate type 3: "precomputed tables are read in ... multi-
+ * dimensional tables are reduced to one-dimensional in T per cell, assuming fixed total mass density and elemental abundances
+ * during thermochemical steps") ----
+ * n_tab tables of ln k on nodes uniform in ln rho (n_rho nodes from ln_rho0, spacing d_ln_rho; n_rho = 1: no density
+ * dependence) and in ln T (n_T nodes from ln_T0, spacing d_ln_T).  For every cell the table is reduced along rho at the cell's
+ * density and the resulting 1-D table is interpolated at the cell's temperature; both steps are piecewise linear in the
+ * logarithms, end values outside the table (readings R32 / R33 of DESIGN.md).  The result is the per-cell rate coefficient the
+ * chemistry step takes as an aux row (KR_F_AUX_UNARY with A = 1: any mass-action order): k_out row t may point straight into
+ * the aux array of kr_thermochem_step_ex.  The rates are those at the cell's T at the START of the step: exact for an
+ * isothermal network; for a network with an energy equation they are frozen over the step (not re-interpolated in the
+ * Newton loop).
+ *   ln_k  DEVICE [n_tab * n_rho * n_T], table t, density node i, temperature node j at (t * n_rho + i) * n_T + j
+ *   rho, T  DEVICE [n_cells] (g cm^-3, K);  k_out  DEVICE [n_tab * n_cells], overwritten
+ * Asynchronous on cuda_stream.  KR_EINVAL on bad sizes / spacings / null pointers, KR_ECUDA without a device. */
+int kr_table_rates(int32_t n_tab, int32_t n_rho, int32_t n_T, double ln_rho0, double d_ln_rho, double ln_T0, double d_ln_T,
+                   const double *ln_k, int64_t n_cells, const double *rho, const double *T, double *k_out, void *cuda_stream);
+
 const char *kr_last_error(void);
 const char *kr_version(void);
 

@@ -28,7 +28,7 @@ EXPORTS = [
     "kr_network_kernel_desc", "kr_network_spec_source", "kr_network_spec_compile", "kr_network_wpc_compile", "kr_network_row_compile", "kr_last_mixed_stats", "kr_thermochem_step", "kr_thermochem_step_ex", "kr_thermochem_step_host", "kr_last_launch_count",
     "kr_layout_cell_to_soa", "kr_layout_soa_to_cell", "kr_math_probe", "kr_measure_fp64_peak", "kr_last_error", "kr_version",
     "kr_recon_create", "kr_recon_destroy", "kr_recon_projector", "kr_advect_species_1d", "kr_raytrace_cartesian",
-    "kr_static_scratch_bytes", "kr_static_setup", "kr_static_max_cells", "kr_thermochem_step_static",
+    "kr_static_scratch_bytes", "kr_static_setup", "kr_static_max_cells", "kr_thermochem_step_static", "kr_table_rates",
 ]
 
 _dp = C.POINTER(C.c_double)
@@ -103,6 +103,8 @@ def load() -> C.CDLL:
     lib.kr_static_max_cells.argtypes = [vp, C.POINTER(C.c_int64)]
     lib.kr_thermochem_step_static.argtypes = [vp, C.c_int64, vp, vp, vp, C.c_double, vp, C.c_int32, vp,
                                               C.POINTER(StepStats), vp]
+    lib.kr_table_rates.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.c_double, C.c_double, C.c_double, C.c_double, vp, C.c_int64,
+                                   vp, vp, vp, vp]
     lib.kr_last_launch_count.argtypes = [vp]
     lib.kr_network_kernel_desc.argtypes = [vp, C.c_char_p, C.c_int64]
     lib.kr_network_spec_source.argtypes = [C.POINTER(NetworkDesc), C.c_char_p, C.c_int64]
@@ -357,6 +359,13 @@ class Network:
                                                 _ptr(aux), n_aux, _ptr(status), C.byref(st) if want_stats else None,
                                                 C.c_void_p(stream or None)))
         return st.as_dict() if want_stats else None
+
+
+def table_rates(ln_k, ln_rho0: float, d_ln_rho: float, ln_T0: float, d_ln_T: float, rho, T, k_out, stream: int = 0) -> None:
+    """kr_table_rates: ln_k device tensor [n_tab, n_rho, n_T]; rho, T [n_cells]; k_out [n_tab, n_cells] (or rows of an aux array)."""
+    n_tab, n_rho, n_T = (int(v) for v in ln_k.shape)
+    _check(load().kr_table_rates(n_tab, n_rho, n_T, float(ln_rho0), float(d_ln_rho), float(ln_T0), float(d_ln_T), _ptr(ln_k),
+                                 int(rho.shape[0]), _ptr(rho), _ptr(T), _ptr(k_out), C.c_void_p(stream or None)))
 
 
 def static_scratch_bytes() -> int:
