@@ -61,7 +61,7 @@ constexpr int oQH = oDQT + (ENERGY ? 8 * R : 0);        // [R]  k_f P' - k_r P''
 constexpr int oMT = oQH + (KRR_ANY_TB ? 8 * R : 0);     // [R]  M_r
 constexpr int oRED = oMT + (KRR_ANY_TB ? 8 * R : 0);    // [8 W + 4] reduction scratch, cell slot, scalars
 constexpr int oPK = oRED + 8 * (8 * W + 4);             // [W][12] per-warp parking slots of the controller state + [6] counters
-constexpr int oKEY = oPK + 8 * (12 * W + 6);            // int[2][W][2] pivot keys of the two warps (double buffered)
+constexpr int oKEY = oPK + 8 * (12 * W + 6);            // Key[2][W] best pivot keys of the two warps (double buffered; W = 2 only)
 #ifndef KRR_RU
 #define KRR_RU 3
 #endif
@@ -536,6 +536,9 @@ struct Elim {
   double myrp, xrp[XRD];                      // reciprocal pivot of the column in which the row was the pivot row ...
   int mycol, xcol[XRD];                       // ... and that column
   Key kw;                                     // the warp's best key for the column being searched
+  Key kwin;                                   // two warps: the better of the two warps' keys ...
+  int wwin;                                   // ... and the warp that holds it (it alone publishes its row)
+  volatile Key* KX;                           // two warps: the key exchange slots
   int khi, kH;                                // search in flight: high word of this lane's key, the warp's largest high word
   unsigned klo;
   double rk;                                  // speculative reciprocal of this lane's candidate
@@ -567,10 +570,27 @@ struct Elim {
     const unsigned L = __reduce_max_sync(0xffffffffu, (khi == kH) ? klo : 0u);
     kw = ((long long)kH << 32) | (long long)L;
   }
+  // two warps per cell: the warps exchange their best keys for column kk (8 bytes each, one named barrier of its own) so
+  // that only the warp that holds the pivot row publishes it.  (Both warps used to publish their candidate -- N / 2 16-byte
+  // stores from one lane each -- and the profile showed the single-lane stores throttled by the shared-memory pipe: 17 % of
+  // all stall samples of config 4, half of them for rows nobody reads.)
+  __device__ __forceinline__ void exchange(int kk) {
+    if (W > 1) {
+      volatile Key* kx = KX + (kk & 1) * W;
+      if (lane == 0) kx[wq] = kw;
+      asm volatile("bar.sync 2, %0;" ::"r"(32 * W) : "memory");
+      const Key ko = kx[1 - wq];
+      const Key k0 = (wq == 0) ? kw : ko, k1 = (wq == 0) ? ko : kw;
+      const bool second = k1 > k0;                         // keys carry the row: they are never equal unless both are -1
+      wwin = second ? 1 : 0;
+      kwin = second ? k1 : k0;
+    }
+  }
   // publication of the warp's winner for column kk: its row (WD entries from the current column on, every earlier update
   // applied), the reciprocal of its current-column entry and the key
   template <int WD>
   __device__ __forceinline__ void publish(int kk) {
+    if (W > 1 && wwin != wq) return;
     const int pw = (kw >= 0) ? (63 - (int)(kw & 63)) : -1;
     double2* URw = URb + ((kk & 1) * W + wq) * URS;
     if (gl == pw) {
@@ -622,12 +642,9 @@ struct Elim {
     double2 tail;
     if (W > 1) {
       G->sync();
-      const double2 t0 = URb[((k & 1) * W + 0) * URS + NC2], t1 = URb[((k & 1) * W + 1) * URS + NC2];
-      const Key k0 = (Key)__double_as_longlong(t0.y), k1 = (Key)__double_as_longlong(t1.y);
-      const bool second = k1 > k0;                           // keys carry the row: they are never equal unless both are -1
-      kbest = second ? k1 : k0;
-      tail = second ? t1 : t0;
-      URw = URb + ((k & 1) * W + (second ? 1 : 0)) * URS;
+      kbest = kwin;
+      URw = URb + ((k & 1) * W + wwin) * URS;
+      tail = URw[NC2];
     } else {
       __syncwarp();
       tail = URw[NC2];
@@ -660,12 +677,12 @@ struct Elim {
     // the search for pivot k + 1 is issued in front of the rest of update k, its second reduction behind the first chunk
     const bool more = k + 1 < N;
     if (more) pick_a(k + 1);
-    if (NP <= 1 && more) pick_b();
+    if (NP <= 1 && more) { pick_b(); exchange(k + 1); }
 #pragma unroll
     for (int j0 = 1; j0 < NP; j0 += 2 * UCH) {
       fetch<WD>(j0 + UCH, URw, ub);
       apply<WD>(j0, l, ua);
-      if (j0 == 1 && more) pick_b();
+      if (j0 == 1 && more) { pick_b(); exchange(k + 1); }
       fetch<WD>(j0 + 2 * UCH, URw, ua);
       apply<WD>(j0 + UCH, l, ub);
     }
@@ -737,12 +754,15 @@ __device__ __forceinline__ bool eliminate(const Cell& c, const Grp& G, double h)
   if (!rows_ok) return false;
 
   E.URb = reinterpret_cast<double2*>(c.d(oUR));
+  E.KX = reinterpret_cast<volatile Key*>(c.base + oKEY);
+  E.kwin = -1; E.wwin = 0;
   E.mycol = -1; E.myrp = 0.0; E.kw = -1; E.rk = 0.0; E.khi = 0; E.kH = 0; E.klo = 0u;
 #pragma unroll
   for (int e = 0; e < XRD; ++e) { E.xcol[e] = -1; E.xrp[e] = 0.0; E.xk[e] = 0.0; if (e >= XR) E.xsc[e] = -1.0; }
 
   E.pick_a(0);
   E.pick_b();
+  E.exchange(0);
   E.template publish<NC>(0);
   E.template segment<0>();
 
