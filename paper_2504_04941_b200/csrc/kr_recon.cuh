@@ -151,28 +151,48 @@ __device__ __forceinline__ void kr_cp_async8(double* smem_dst, const double* gme
 __device__ __forceinline__ void kr_cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void kr_cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
+__device__ __forceinline__ void kr_cp_async16(double* smem_dst, const double* gmem_src) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+
 // Persistent blocks walk the tiles with a stride of gridDim.x; the abundances of the NEXT tile are already on their way
-// into the second staging buffer (cp.async) while the current tile is limited, projected and updated, so that the HBM
-// reads overlap the arithmetic instead of alternating with it.
+// into the second staging buffer (cp.async, 16 bytes per request where the field allows) while the current tile is
+// limited, projected and updated, so that the HBM reads overlap the arithmetic instead of alternating with it.
+// A block of T threads owns T - 2 cells: the update of a tile needs the corrections of its cells and of one halo cell on
+// each side, T values, so thread t forms the correction of cell c0 - 1 + t -- one pass for every thread (with T cells per
+// tile the two halo corrections cost the whole first warp a second pass, and the block waited for it at the barrier).
+// Two block barriers per tile: the tile has landed / the corrections are written.  The results are staged per WARP (a
+// warp's 32 cells are one contiguous range of the output) and written out coalesced behind a warp-level sync.
 template <int S>
-struct KrAdvectTile { static constexpr int T = (S <= 10) ? 128 : 64; };   // 48 KiB of static shared memory
+struct KrAdvectTile { static constexpr int T = (S <= 10) ? 128 : 64; static constexpr int TO = T - 2; };   // < 48 KiB of static shared memory
 
 template <int S>
 __global__ void __launch_bounds__(KrAdvectTile<S>::T) kr_advect_cell_kernel(const KrAdvectArgsP<S> ap) {
-  constexpr int T = KrAdvectTile<S>::T, LDY = S | 1; // cells per tile = threads per block; padded row: conflict-free 64-bit accesses
+  constexpr int T = KrAdvectTile<S>::T, TO = KrAdvectTile<S>::TO, LDY = S | 1;   // padded row: conflict-free 64-bit accesses
   const KrAdvectArgs& a = ap.a;
-  __shared__ double sybuf[2][(T + 4) * LDY];         // cells c0 - 2 .. c0 + T + 1, double buffered
-  __shared__ double sd[(T + 2) * LDY];               // corrections of cells c0 - 1 .. c0 + T; later the results of the tile
-  const int tid = threadIdx.x;
-  const long long n_tiles = (a.n_cells + T - 1) / T;
+  __shared__ __align__(16) double sybuf[2][(T + 2) * LDY];   // cells c0 - 2 .. c0 + TO + 1, double buffered
+  __shared__ __align__(16) double sd[T * LDY];               // corrections of cells c0 - 1 .. c0 + TO
+  __shared__ __align__(16) double so[T * LDY];               // results of the tile, rows of a warp written and read by that warp only
+  const int tid = threadIdx.x, lane = tid & 31, w0 = tid & ~31;
+  const long long n_tiles = (a.n_cells + TO - 1) / TO;
 
   auto stage = [&](long long tile, double* sy) {      // asynchronous, coalesced copy of tile + halo into sy
-    const long long c0 = tile * T;
-    const int nt = (int)min((long long)T, a.n_cells - c0);
+    const long long c0 = tile * TO;
+    const int nt = (int)min((long long)TO, a.n_cells - c0);
     if (c0 >= 2 && c0 + nt + 2 <= a.n_cells) {
       const double* src = a.y + (c0 - 2) * S;
-      if (LDY == S) { for (int i = tid; i < (nt + 4) * S; i += T) kr_cp_async8(sy + i, src + i); }
-      else { for (int i = tid; i < (nt + 4) * S; i += T) kr_cp_async8(sy + (i / S) * LDY + (i % S), src + i); }
+      const int cnt = (nt + 4) * S;
+      if (LDY == S) {
+        if ((reinterpret_cast<unsigned long long>(src) & 15ull) == 0ull) {      // c0 is even: true whenever a.y is 16-byte aligned
+          for (int i = tid; i < cnt / 2; i += T) kr_cp_async16(sy + 2 * i, src + 2 * i);
+          if ((cnt & 1) && tid == 0) kr_cp_async8(sy + cnt - 1, src + cnt - 1);
+        } else {
+          for (int i = tid; i < cnt; i += T) kr_cp_async8(sy + i, src + i);
+        }
+      } else {
+        for (int i = tid; i < cnt; i += T) kr_cp_async8(sy + (i / S) * LDY + (i % S), src + i);
+      }
     } else {
       for (int i = tid; i < (nt + 4) * S; i += T) {
         const int cl = i / S, s = i % S;
@@ -186,13 +206,13 @@ __global__ void __launch_bounds__(KrAdvectTile<S>::T) kr_advect_cell_kernel(cons
   if ((long long)blockIdx.x < n_tiles) stage(blockIdx.x, sybuf[0]);
   for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, buf ^= 1) {
     const double* sy = sybuf[buf];
-    const long long c0 = tile * T;
-    const int nt = (int)min((long long)T, a.n_cells - c0);
+    const long long c0 = tile * TO;
+    const int nt = (int)min((long long)TO, a.n_cells - c0);
     kr_cp_async_wait_all();
     __syncthreads();                                  // the tile is in sy; everybody is done with the other buffer and with sd
     if (tile + gridDim.x < n_tiles) stage(tile + gridDim.x, sybuf[buf ^ 1]);
     // the cell's scalars are requested now, so that their latency hides under the corrections
-    const int cl = tid;
+    const int cl = tid;                               // thread <-> cell c0 + cl of the update, correction of cell c0 - 1 + cl
     double fl = 0.0, fr = 0.0, rho = 1.0, r0 = 0.0;
     if (cl < nt) {
       const long long c = c0 + cl;
@@ -202,7 +222,7 @@ __global__ void __launch_bounds__(KrAdvectTile<S>::T) kr_advect_cell_kernel(cons
       if (a.y0) r0 = a.rho0[c];
     }
     // corrections of cells c0 - 1 .. c0 + nt: limited half-differences (eqs. 10-12), projected (eq. 13)
-    for (int cl = tid; cl < nt + 2; cl += T) {
+    if (cl < nt + 2) {
       double g[S];
       if (a.scheme == KR_RECON_DONOR) {
 #pragma unroll
@@ -228,8 +248,7 @@ __global__ void __launch_bounds__(KrAdvectTile<S>::T) kr_advect_cell_kernel(cons
       }
     }
     __syncthreads();
-    // conservative update of the tile (eq. 1, eq. 14, step 3 of PAPER.md:40); results staged for a coalesced write
-    double out[S];
+    // conservative update of the tile (eq. 1, eq. 14, step 3 of PAPER.md:40); results staged per warp for a coalesced write
     if (cl < nt) {
       const long long c = c0 + cl;
       double rn = rho - a.lambda * (fr - fl);
@@ -244,18 +263,27 @@ __global__ void __launch_bounds__(KrAdvectTile<S>::T) kr_advect_cell_kernel(cons
         const double yr = rup ? yc + dc : sy[(cl + 3) * LDY + s] - sd[(cl + 2) * LDY + s];
         double un = rho * yc - a.lambda * (yr * fr - yl * fl);
         if (a.y0) un = a.wa * r0 * a.y0[c * S + s] + a.wb * un;
-        out[s] = un * rinv;
+        so[cl * LDY + s] = un * rinv;
       }
     }
-    __syncthreads();                                  // every thread has read sd
-    if (cl < nt) {
-#pragma unroll
-      for (int s = 0; s < S; ++s) sd[cl * LDY + s] = out[s];
+    __syncwarp();
+    {                                                 // the warp's cells c0 + w0 .. : one contiguous range of y_out
+      const int nw = min(32, nt - w0);                // may be <= 0
+      double* dst = a.y_out + (c0 + w0) * S;
+      const double* src = so + w0 * LDY;
+      if (LDY == S) {
+        if ((reinterpret_cast<unsigned long long>(dst) & 15ull) == 0ull) {
+          const int cnt = nw * S;
+          for (int i = lane; i < cnt / 2; i += 32) reinterpret_cast<double2*>(dst)[i] = reinterpret_cast<const double2*>(src)[i];
+          if ((cnt & 1) && lane == 0) dst[cnt - 1] = src[cnt - 1];
+        } else {
+          for (int i = lane; i < nw * S; i += 32) dst[i] = src[i];
+        }
+      } else {
+        for (int i = lane; i < nw * S; i += 32) dst[i] = src[(i / S) * LDY + (i % S)];
+      }
     }
-    __syncthreads();
-    double* dst = a.y_out + c0 * S;
-    if (LDY == S) { for (int i = tid; i < nt * S; i += T) dst[i] = sd[i]; }
-    else { for (int i = tid; i < nt * S; i += T) dst[i] = sd[(i / S) * LDY + (i % S)]; }
+    __syncwarp();                                     // the warp's rows of so are free again
   }
 }
 
@@ -271,9 +299,9 @@ inline cudaError_t kr_advect_cell_launch(const KrAdvectArgs& a, const double* P_
     cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
   }
   int per_sm = 0;
-  constexpr int T = KrAdvectTile<S>::T;
+  constexpr int T = KrAdvectTile<S>::T, TO = KrAdvectTile<S>::TO;
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kr_advect_cell_kernel<S>, T, 0);
-  const long long n_tiles = (a.n_cells + T - 1) / T;
+  const long long n_tiles = (a.n_cells + TO - 1) / TO;
   const unsigned grid = unsigned(std::min<long long>(n_tiles, (long long)std::max(1, per_sm) * std::max(1, n_sm)));
   kr_advect_cell_kernel<S><<<grid, T, 0, st>>>(ap);
   return cudaGetLastError();
