@@ -53,6 +53,28 @@ def test_table_rates_match_oracle(B, n_rho, n_T, n_cells):
     assert np.all(k_gpu[tiny] < 1e-299)
 
 
+@pytest.mark.parametrize("n_rho,n_T", [(1, 4097), (3, 1024)])
+def test_table_rates_staged_path_matches_oracle(B, n_rho, n_T):
+    """Batches of at least 1024 cells per SM take the kernel that stages the tables in shared memory (tables <= 200 KiB):
+    the same values as the global-memory path and as the oracle, the latter on a seeded sample of the cells."""
+    from oracle import table_oracle as TO
+    net, _, _ = w.make_config(2, 8)
+    table = w.make_rate_table(net, [0, 1, 3, 4, 6, 7], T_range=(50.0, 2.0e5), n_T=n_T, n_rho=n_rho, rho_exponent=0.37)
+    assert table.ln_k.size * 8 <= 200 * 1024
+    n_cells = 400_003                                      # > 1024 cells per SM on any part, ragged
+    rng = np.random.default_rng(4242)
+    T = np.exp(rng.uniform(math.log(20.0), math.log(5.0e5), n_cells))
+    rho = np.exp(rng.uniform(math.log(1e-26), math.log(1e-12), n_cells))
+    k_big = _gpu_rates(B, table, rho, T)
+    assert np.all(np.isfinite(k_big)) and np.all(k_big >= 0.0)
+    sample = np.concatenate([np.arange(64), rng.choice(n_cells, 3000, replace=False), np.arange(n_cells - 64, n_cells)])
+    k_small = _gpu_rates(B, table, rho[sample], T[sample])              # 3 128 cells: the global-memory path
+    np.testing.assert_array_equal(k_big[:, sample], k_small)
+    k_ref = TO.table_rates(table.ln_k, table.ln_rho0, table.d_ln_rho, table.ln_T0, table.d_ln_T, rho[sample], T[sample])
+    tiny = k_ref < 1e-300
+    np.testing.assert_allclose(k_small[~tiny], k_ref[~tiny], rtol=1e-10, atol=0.0)
+
+
 def test_empty_and_bad_arguments(B):
     import torch
     dev = "cuda:0"
