@@ -526,6 +526,9 @@ constexpr int seg_lo(int i) { return (int)((long long)i * N / SEG); }
 #ifndef KRR_UCH
 #define KRR_UCH 6
 #endif
+#ifndef KRR_EARLY_PUB
+#define KRR_EARLY_PUB 1
+#endif
 constexpr int UCH = KRR_UCH;                  // pairs of the pivot row per chunk (two chunks in flight)
 
 struct Elim {
@@ -588,14 +591,14 @@ struct Elim {
   }
   // publication of the warp's winner for column kk: its row (WD entries from the current column on, every earlier update
   // applied), the reciprocal of its current-column entry and the key
-  template <int WD>
+  template <int WD, int FROM = 0>
   __device__ __forceinline__ void publish(int kk) {
     if (W > 1 && wwin != wq) return;
     const int pw = (kw >= 0) ? (63 - (int)(kw & 63)) : -1;
     double2* URw = URb + ((kk & 1) * W + wq) * URS;
     if (gl == pw) {
 #pragma unroll
-      for (int j = 0; j < (WD + 1) / 2; ++j) URw[j] = a[j];
+      for (int j = FROM; j < (WD + 1) / 2; ++j) URw[j] = a[j];
       URw[NC2] = make_double2(rk, __longlong_as_double((long long)kw));
     }
 #pragma unroll
@@ -609,6 +612,20 @@ struct Elim {
         if (lane == 0) URw[NC2] = make_double2(krs_rcp(xk[e]), __longlong_as_double((long long)kw));
       }
     if (W > 1 && pw < 0 && lane == 0) URw[NC2] = make_double2(0.0, __longlong_as_double(-1LL));   // no candidate in this warp
+  }
+
+  // Early publication: the pivot row of the NEXT column is named while the update of this column has hardly begun, so the
+  // lane that holds it stores every chunk of its row as soon as the chunk is updated instead of all of it behind the update
+  // (N / 2 back-to-back 16-byte stores from one lane fill the queue of the shared-memory pipe -- mio throttle was 17 % of
+  // the stall samples of config 4 -- and the rest of the group waits for the last of them).  Pairs lo .. hi of the row as it
+  // will stand for the next column; fin is the last pair an update chunk completes.
+  template <int WDN>
+  __device__ __forceinline__ void pub_pairs(double2* URn, bool pubme, int lo, int hi, int fin) {
+#pragma unroll
+    for (int q = 0; q < UCH; ++q) {
+      const int pp = lo + q;
+      if (pp <= hi && pp <= fin && pp < (WDN + 1) / 2) { if (pubme) URn[pp] = a[pp]; }
+    }
   }
 
   // update of the pairs j0 .. j0 + UCH - 1 of the shifted row from the chunk u: entries 2j, 2j + 1 -> 2j - 1, 2j
@@ -678,15 +695,23 @@ struct Elim {
     const bool more = k + 1 < N;
     if (more) pick_a(k + 1);
     if (NP <= 1 && more) { pick_b(); exchange(k + 1); }
+    constexpr int FIN = NP - 2;                              // new pair p is complete once the chunk with old pair p + 1 is applied
+    bool pubme = false;
+    double2* URn = URb + (((k + 1) & 1) * W + wq) * URS;
 #pragma unroll
     for (int j0 = 1; j0 < NP; j0 += 2 * UCH) {
       fetch<WD>(j0 + UCH, URw, ub);
       apply<WD>(j0, l, ua);
-      if (j0 == 1 && more) { pick_b(); exchange(k + 1); }
+      if (j0 == 1 && more) {
+        pick_b(); exchange(k + 1);
+        pubme = (KRR_EARLY_PUB != 0) && (kw >= 0) && (gl == 63 - (int)(kw & 63)) && (W == 1 || wwin == wq);
+      }
+      if (KRR_EARLY_PUB && more) pub_pairs<WD - 1>(URn, pubme, j0 == 1 ? 0 : j0 - 1, j0 + UCH - 2, FIN);
       fetch<WD>(j0 + 2 * UCH, URw, ua);
       apply<WD>(j0 + UCH, l, ub);
+      if (KRR_EARLY_PUB && more) pub_pairs<WD - 1>(URn, pubme, j0 + UCH - 1, j0 + 2 * UCH - 2, FIN);
     }
-    if (more) publish<WD - 1>(k + 1);
+    if (more) publish<WD - 1, (KRR_EARLY_PUB && FIN >= 0) ? FIN + 1 : 0>(k + 1);
   }
 
   template <int SI>

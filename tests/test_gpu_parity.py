@@ -112,11 +112,11 @@ def test_parity_mixed_precision(B, oracle_mod, idx, fixed):
     assert stats["n_newton"] <= 1.6 * ref["stats"]["n_newton"] + 50
 
 
-@pytest.mark.parametrize("S,energy,n_rev,mode", [(13, 1, 10, 0), (24, 0, 90, 0), (24, 0, 90, 1), (40, 1, 150, 0), (47, 1, 200, 0),
+@pytest.mark.parametrize("S,energy,n_rev,mode", [(13, 1, 10, 0), (24, 0, 90, 0), (24, 0, 90, 1), (32, 0, 120, 0), (33, 1, 120, 0), (40, 1, 150, 0), (47, 1, 200, 0),
                                                   (63, 1, 260, 0), (63, 1, 260, 1), (64, 1, 260, 0)])
 def test_register_tile_kernel_on_other_sizes(B, oracle_mod, S, energy, n_rev, mode):
     """Sizes between the BASELINE configs: every tile shape the host can pick (one warp up to 48 doubles per thread, two
-    warps above, the energy equation on a warp pair, N = 64 and N = 65 -> shared-memory kernel) against the oracle, fp64
+    warps above; N = 32: a full warp of rows, N = 34: two rows spread over the lanes of the row-per-lane kernel, the energy equation on a warp pair, N = 64 and N = 65 -> shared-memory kernel) against the oracle, fp64
     and mixed, on seeded astro-like networks of the config-3 recipe."""
     rng = np.random.default_rng(4242 + 100 * S + energy)
     net = w._network_random(rng, 3, 5, S, n_rev, 10, 10, energy, reversible=False)
