@@ -138,6 +138,8 @@ __global__ void __launch_bounds__(128) kr_advect_kernel(const KrAdvectArgs a) {
 // constant bank, so each of the S^2 products of eq. 13 is ONE DFMA with a constant-bank operand -- no load, no index.
 #define KR_RECON_SMAX 16
 
+template <bool V> struct KrBool { static constexpr bool value = V; };
+
 template <int S>
 struct KrAdvectArgsP {
   KrAdvectArgs a;
@@ -256,15 +258,23 @@ __global__ void __launch_bounds__(KrAdvectTile<S>::T) kr_advect_cell_kernel(cons
       const double rinv = krs_rcp(rn);
       if (a.rho_out) a.rho_out[c] = rn;
       const bool lup = fl > 0.0, rup = fr > 0.0;
+      // eq. 14: the upwind side of each face.  One code path per pair of directions, so that only the operands of the
+      // sides that are used are read from shared memory (2 to 6 loads per species; the flow direction is coherent over
+      // long stretches of cells, so the lanes of a warp mostly agree)
+      auto update = [&](auto LUP, auto RUP) {
 #pragma unroll
-      for (int s = 0; s < S; ++s) {
-        const double yc = sy[(cl + 2) * LDY + s], dc = sd[(cl + 1) * LDY + s];
-        const double yl = lup ? sy[(cl + 1) * LDY + s] + sd[cl * LDY + s] : yc - dc;
-        const double yr = rup ? yc + dc : sy[(cl + 3) * LDY + s] - sd[(cl + 2) * LDY + s];
-        double un = rho * yc - a.lambda * (yr * fr - yl * fl);
-        if (a.y0) un = a.wa * r0 * a.y0[c * S + s] + a.wb * un;
-        so[cl * LDY + s] = un * rinv;
-      }
+        for (int s = 0; s < S; ++s) {
+          const double yc = sy[(cl + 2) * LDY + s], dc = sd[(cl + 1) * LDY + s];
+          double yl, yr;
+          if constexpr (decltype(LUP)::value) yl = sy[(cl + 1) * LDY + s] + sd[cl * LDY + s]; else yl = yc - dc;
+          if constexpr (decltype(RUP)::value) yr = yc + dc; else yr = sy[(cl + 3) * LDY + s] - sd[(cl + 2) * LDY + s];
+          double un = rho * yc - a.lambda * (yr * fr - yl * fl);
+          if (a.y0) un = a.wa * r0 * a.y0[c * S + s] + a.wb * un;
+          so[cl * LDY + s] = un * rinv;
+        }
+      };
+      if (lup) { if (rup) update(KrBool<true>{}, KrBool<true>{}); else update(KrBool<true>{}, KrBool<false>{}); }
+      else { if (rup) update(KrBool<false>{}, KrBool<true>{}); else update(KrBool<false>{}, KrBool<false>{}); }
     }
     __syncwarp();
     {                                                 // the warp's cells c0 + w0 .. : one contiguous range of y_out
