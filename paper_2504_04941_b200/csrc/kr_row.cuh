@@ -67,7 +67,7 @@ constexpr int oKEY = oPK + 8 * (12 * W + 6);            // Key[2][W] best pivot 
 #endif
 constexpr int RU = KRR_RU;                              // reactions in flight per thread (reactions())
 #ifndef KRR_SB
-#define KRR_SB 8
+#define KRR_SB 4      // measured (full size): 8 -> 4 steps per batch c3 -2.9 %, c4 -3.2 %; 2: c4 +9 %
 #endif
 constexpr int SB = KRR_SB;                              // steps per batch of the term streams (the host pads to it)
 constexpr int NSLOT = KRR_NSLOT;                        // partial sums of the row program (host-built chunks)
@@ -519,12 +519,12 @@ __device__ __forceinline__ Key key_of(double v, double sc, int row) {
 constexpr int XRD = XR > 0 ? XR : 1;
 constexpr int URS = NC2 + 1;                  // one published row: NC2 pairs + {reciprocal of its column-k entry, its key}
 #ifndef KRR_SEG
-#define KRR_SEG 8
+#define KRR_SEG (KRR_N >= 64 ? 16 : 8)      // measured on N = 64: 16 segments -2.5 % (less dead width per column), 4: +6 %; N = 33: 4 +2 %, 11 +21 %
 #endif
 constexpr int SEG = (N >= 4 * KRR_SEG) ? KRR_SEG : 1;
 constexpr int seg_lo(int i) { return (int)((long long)i * N / SEG); }
 #ifndef KRR_UCH
-#define KRR_UCH 6
+#define KRR_UCH (KRR_W == 1 ? 2 : 4)      // measured (full size): two warps 6 -> 4 pairs per chunk -3 %; one warp 6 -> 2 with 12 instead of 8 cells per SM -2.3 % on top of -4 % from the batches; 8: +2.5 %
 #endif
 #ifndef KRR_EARLY_PUB
 #define KRR_EARLY_PUB 1
