@@ -364,6 +364,47 @@ def bench_advection(args, ctx) -> dict:
             "note": "the step before the chemistry step in the paper's cycle (PAPER.md section 2.1); input larger than L2 and L2 flushed between launches"}
 
 
+def bench_raytrace(args, ctx) -> dict:
+    """kr_raytrace_cartesian (section 3, eqs. 24, 29-31) on config 2's mesh (256^3 cells): one
+    plane-parallel ray along +x through every (y, z) column (the plane-parallel source of PAPER.md Fig. 2), two absorbers,
+    four energy bins.  Algorithmic bytes: every cell's absorber densities read once and its rate coefficients written once
+    (16 B per absorber and cell) plus the rays; the call also zeroes the rate field first (inside the timed region)."""
+    import torch
+    from paper_2504_04941_b200 import binding as B
+    dev = ctx["dev"]
+    nx = ny = nz = args.ray_mesh
+    n_abs, n_bins = 2, 4
+    case = w.make_ray_case(shape=(nx, ny, nz), n_oblique=0, n_abs=n_abs, n_bins=n_bins, seed=w.BASE_SEED + 3001, columns=True)
+    t = lambda a: torch.tensor(np.ascontiguousarray(a), device=dev)
+    nd = t(case["n_dens"].reshape(n_abs, -1)); k = torch.empty_like(nd)
+    org, drc, L = t(case["origins"]), t(case["directions"]), t(case["L"])
+    Lo = torch.empty_like(L); path = torch.empty(org.shape[0], dtype=torch.float64, device=dev)
+    n_rays, n_cells = int(org.shape[0]), nx * ny * nz
+    stream = torch.cuda.current_stream()
+    run = lambda: B.raytrace_cartesian(case["shape"], case["spacing"], n_rays, org, drc, L, case["sigma"], nd, k, Lo, path,
+                                       stream=stream.cuda_stream)
+    for _ in range(3):
+        run()
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for a, b in ev:
+        ctx["flush"].zero_()
+        a.record(stream); run(); b.record(stream)
+    torch.cuda.synchronize()
+    ms = float(np.mean([a.elapsed_time(b) for a, b in ev]))
+    assert abs(float(path.min().item()) - nx * case["spacing"][0]) < 1e-9          # every ray crossed the whole mesh
+    bytes_launch = float(n_cells) * 16 * n_abs + float(n_rays) * 8 * (6 + 2 * n_bins + 1)
+    peak, src = hbm_peak()
+    gbs = bytes_launch / (ms * 1e-3) / 1e9
+    return {"workload": f"raytrace_cartesian_{nx}x{ny}x{nz}_abs{n_abs}_bins{n_bins}", "dtype": "f64", "cells": n_cells, "rays": n_rays,
+            "value": n_cells / (ms * 1e-3), "unit": "cell-crossings/s", "ms_per_launch": ms, "gpu_launches": args.steps,
+            "roofline": {"bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak, "traffic": None,
+                         "traffic_note": TRAFFIC_NOTE, "peak_source": src, "bytes_per_launch": bytes_launch},
+            "note": "the photo-reaction rate field that feeds config 2's chemistry step (PAPER.md section 3); per cell crossing "
+                    "and energy bin one exp() and one expm1() in FP64, three FP64 divides per crossing (eq. 24 un-contracted, so "
+                    "that the visited cells equal the oracle's); mesh larger than L2 and L2 flushed between launches"}
+
+
 def bench_table_rates(args, ctx) -> dict:
     """kr_table_rates for config 2's six thermal rate laws read from tables (n_rho = 1,
     4 097 temperature nodes: 197 KB of table, resident in L2), on 2^24 cells with config 2's temperature and density
@@ -420,7 +461,7 @@ def worker(args, rank: int, local_rank: int, world: int) -> None:
                peak_tf=B.measure_fp64_peak(8192))
     if args.advection_only:
         if rank == 0:
-            print(json.dumps({"next": {"advection": bench_advection(args, ctx), "table_rates": bench_table_rates(args, ctx)}}), flush=True)
+            print(json.dumps({"next": {"advection": bench_advection(args, ctx), "raytrace": bench_raytrace(args, ctx), "table_rates": bench_table_rates(args, ctx)}}), flush=True)
         return
     if args.config is not None:
         runs = [(args.config, args.mode)]
@@ -435,6 +476,7 @@ def worker(args, rank: int, local_rank: int, world: int) -> None:
     advection = None
     if rank == 0 and world == 1 and args.config is None and not args.no_advection:
         advection = bench_advection(args, ctx)
+        raytrace = bench_raytrace(args, ctx)
         table_rates = bench_table_rates(args, ctx)
     if rank == 0:
         head = next((r for r, (i, m) in zip(results, runs) if i == HEADLINE and m == "fp64"), results[0])
@@ -452,7 +494,7 @@ def worker(args, rank: int, local_rank: int, world: int) -> None:
                                 "notes": r["config"]["notes"]} for r in results]
             line["gpu_launches"] = int(sum(r["gpu_launches"] for r in results))
         if advection is not None:
-            line["next"] = {"advection": advection, "table_rates": table_rates}
+            line["next"] = {"advection": advection, "raytrace": raytrace, "table_rates": table_rates}
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
@@ -483,6 +525,7 @@ def main() -> None:
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-advection", action="store_true", help="skip the NEXT-2 advection-stage bandwidth measurement")
     ap.add_argument("--advect-cells", type=int, default=1 << 24)
+    ap.add_argument("--ray-mesh", type=int, default=256, help="cells per side of the NEXT-3 ray-tracing mesh (config 2's: 256)")
     ap.add_argument("--advection-only", action="store_true", help="measure only the NEXT-2 advection stage (profiling runs)")
     args = ap.parse_args()
     under_launcher = "RANK" in os.environ and "WORLD_SIZE" in os.environ

@@ -23,18 +23,52 @@ struct KrRayArgs {
   double sigma[KR_RAY_MAX_ABS * KR_RAY_MAX_BINS];   // [n_abs][n_bins]
 };
 
-// (1 - exp(-tau)) / tau of eqs. 28 and 30 (reading R30)
-__device__ __forceinline__ double kr_thin_factor(double tau) { return (tau == 0.0) ? 1.0 : -expm1(-tau) / tau; }
+// exp(x) and expm1(x) for x <= 0 from ONE reduction and ONE polynomial (eqs. 28-30 need both in every cell and energy bin:
+// the attenuation exp(-tau) and, reading R30, (1 - exp(-tau)) / tau as -expm1(-tau) / tau).  x = n ln 2 + r, |r| <= ln 2 / 2;
+// p = expm1(r) as r times a degree-12 Taylor polynomial; exp = 2^n + 2^n p, expm1 = (2^n - 1) + 2^n p, both one FMA on exact
+// operands: <= 1.8e-16 / 2.8e-16 relative against long-double exp / expm1 on 3e7 arguments in [-700, -1e-12].  Below -708
+// the pair is (0, -1) (the attenuated photon count there is < 1e-307 of the incoming one).
+__device__ __forceinline__ void kr_exp_pair(double x, double& e, double& m) {
+  const double t = fma(x, 1.4426950408889634074, 6755399441055744.0);
+  const int n = __double2loint(t);
+  const double fn = t - 6755399441055744.0;
+  double r = fma(fn, -6.93147180369123816490e-01, x);
+  r = fma(fn, -1.90821492927058770002e-10, r);
+  double p = 1.0 / 6227020800.0;
+  p = fma(p, r, 1.0 / 479001600.0);
+  p = fma(p, r, 1.0 / 39916800.0);
+  p = fma(p, r, 1.0 / 3628800.0);
+  p = fma(p, r, 1.0 / 362880.0);
+  p = fma(p, r, 1.0 / 40320.0);
+  p = fma(p, r, 1.0 / 5040.0);
+  p = fma(p, r, 1.0 / 720.0);
+  p = fma(p, r, 1.0 / 120.0);
+  p = fma(p, r, 1.0 / 24.0);
+  p = fma(p, r, 1.0 / 6.0);
+  p = fma(p, r, 0.5);
+  p = fma(p, r, 1.0);
+  p = p * r;
+  const double s = __hiloint2double((1023 + n) << 20, 0);      // 2^n, -1022 <= n <= 0
+  const bool tiny = x < -708.0;
+  e = tiny ? 0.0 : fma(s, p, s);
+  m = tiny ? -1.0 : fma(s, p, s - 1.0);
+}
 
+// NA, NB > 0: the numbers of absorbers and energy bins are compile-time constants (every per-cell array is then a set of
+// registers; with run-time bounds they are local-memory arrays); 0: run-time bounds up to the maxima.
+template <int NA, int NB>
 __global__ void __launch_bounds__(128) kr_raytrace_kernel(const KrRayArgs a) {
+  constexpr int MA = NA > 0 ? NA : KR_RAY_MAX_ABS, MB = NB > 0 ? NB : KR_RAY_MAX_BINS;
+  const int n_abs = NA > 0 ? NA : a.n_abs, n_bins = NB > 0 ? NB : a.n_bins;
   const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= a.n_rays) return;
   const int n[3] = {a.nx, a.ny, a.nz};
   double d[3] = {a.dirs[3 * j], a.dirs[3 * j + 1], a.dirs[3 * j + 2]};
   const double o[3] = {a.origins[3 * j], a.origins[3 * j + 1], a.origins[3 * j + 2]};
   const double norm = sqrt(__dadd_rn(__dadd_rn(__dmul_rn(d[0], d[0]), __dmul_rn(d[1], d[1])), __dmul_rn(d[2], d[2])));
-  double L[KR_RAY_MAX_BINS];
-  for (int b = 0; b < a.n_bins; ++b) L[b] = a.L_in[j * a.n_bins + b];
+  double L[MB];
+#pragma unroll
+  for (int b = 0; b < MB; ++b) L[b] = (b < n_bins) ? a.L_in[j * n_bins + b] : 0.0;
   double total = 0.0;
   // entry into the mesh: slab method
   double t0 = 0.0, t1 = __longlong_as_double(0x7ff0000000000000LL);
@@ -77,19 +111,27 @@ __global__ void __launch_bounds__(128) kr_raytrace_kernel(const KrRayArgs a) {
       const long long cell = ((long long)idx[0] * a.ny + idx[1]) * a.nz + idx[2];
       total += dl;
       // eqs. 29-31 in this cell
-      double nd[KR_RAY_MAX_ABS];
-      for (int i = 0; i < a.n_abs; ++i) nd[i] = a.n_dens[(long long)i * a.n_cells + cell];
-      double add[KR_RAY_MAX_ABS];
-      for (int i = 0; i < a.n_abs; ++i) add[i] = 0.0;
-      for (int b = 0; b < a.n_bins; ++b) {
-        double tau = 0.0;
-        for (int i = 0; i < a.n_abs; ++i) tau += nd[i] * a.sigma[i * a.n_bins + b] * dl;
-        const double f = kr_thin_factor(tau);
-        for (int i = 0; i < a.n_abs; ++i) add[i] += L[b] * a.sigma[i * a.n_bins + b] * dl * inv_dV * f;
-        L[b] *= exp(-tau);
-      }
-      for (int i = 0; i < a.n_abs; ++i)
-        if (add[i] != 0.0) atomicAdd(a.k_out + (long long)i * a.n_cells + cell, add[i]);
+      double nd[MA], add[MA];
+#pragma unroll
+      for (int i = 0; i < MA; ++i) { nd[i] = (i < n_abs) ? a.n_dens[(long long)i * a.n_cells + cell] : 0.0; add[i] = 0.0; }
+#pragma unroll
+      for (int b = 0; b < MB; ++b)
+        if (b < n_bins) {
+          double tau = 0.0;
+#pragma unroll
+          for (int i = 0; i < MA; ++i)
+            if (i < n_abs) tau += nd[i] * a.sigma[i * n_bins + b] * dl;
+          double e, m;
+          kr_exp_pair(-tau, e, m);
+          const double f = (tau == 0.0) ? 1.0 : -m / tau;          // (1 - exp(-tau)) / tau of eqs. 28 and 30 (reading R30)
+#pragma unroll
+          for (int i = 0; i < MA; ++i)                             // in this order: deep inside an absorber L sigma is subnormal
+            if (i < n_abs) add[i] += L[b] * a.sigma[i * n_bins + b] * dl * inv_dV * f;
+          L[b] *= e;
+        }
+#pragma unroll
+      for (int i = 0; i < MA; ++i)
+        if (i < n_abs && add[i] != 0.0) atomicAdd(a.k_out + (long long)i * a.n_cells + cell, add[i]);
       // leave through every surface reached at dl (edges and corners: several at once)
 #pragma unroll
       for (int c = 0; c < 3; ++c) {
@@ -102,6 +144,10 @@ __global__ void __launch_bounds__(128) kr_raytrace_kernel(const KrRayArgs a) {
       }
     }
   }
-  if (a.L_out) for (int b = 0; b < a.n_bins; ++b) a.L_out[j * a.n_bins + b] = L[b];
+  if (a.L_out) {
+#pragma unroll
+    for (int b = 0; b < MB; ++b)
+      if (b < n_bins) a.L_out[j * n_bins + b] = L[b];
+  }
   if (a.path) a.path[j] = total;
 }
