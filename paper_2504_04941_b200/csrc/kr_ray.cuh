@@ -5,6 +5,7 @@
 // through FP64 atomic adds (the sum over j in eq. 31); with one ray per cell (plane-parallel rays along a mesh axis)
 // every cell has a single writer.  Cross sections travel in the parameter block (constant bank).
 #pragma once
+#include "kr_math.cuh"
 
 #define KR_RAY_MAX_ABS 8
 #define KR_RAY_MAX_BINS 16
@@ -97,23 +98,35 @@ __global__ void __launch_bounds__(128) kr_raytrace_kernel(const KrRayArgs a) {
     }
     const double inv_dV = 1.0 / (a.h[0] * a.h[1] * a.h[2]);
     const int limit = a.nx + a.ny + a.nz + 3;
+    // the absorber densities of a cell are requested as soon as the walk knows the cell -- at the end of the step before --
+    // so that their latency hides under eq. 24 of the step that uses them
+    double nd[MA];
+    auto request = [&]() {
+      const bool in = !(idx[0] < 0 || idx[0] >= n[0] || idx[1] < 0 || idx[1] >= n[1] || idx[2] < 0 || idx[2] >= n[2]);
+      const long long cn = in ? ((long long)idx[0] * a.ny + idx[1]) * a.nz + idx[2] : 0;
+#pragma unroll
+      for (int i = 0; i < MA; ++i) nd[i] = (in && i < n_abs) ? __ldg(a.n_dens + (long long)i * a.n_cells + cn) : 0.0;
+    };
+    request();
     for (int step = 0; step < limit; ++step) {
       if (idx[0] < 0 || idx[0] >= n[0] || idx[1] < 0 || idx[1] >= n[1] || idx[2] < 0 || idx[2] >= n[2]) break;
       // eq. 24: 0 = x_d dl + (x_in - x_int) for the three surfaces on the side of the direction
       double dls[3];
 #pragma unroll
       for (int c = 0; c < 3; ++c) {
-        if (d[c] > 0.0) dls[c] = (__dadd_rn(a.lo[c], __dmul_rn((double)(idx[c] + 1), a.h[c])) - x[c]) / d[c];
-        else if (d[c] < 0.0) dls[c] = (__dadd_rn(a.lo[c], __dmul_rn((double)idx[c], a.h[c])) - x[c]) / d[c];
+        // (a component of +-1 -- a ray along a mesh axis -- divides exactly: the product is the same number without the
+        // FP64 divide, which is a ~25-instruction routine on this chip)
+        if (d[c] > 0.0) { const double df = __dadd_rn(a.lo[c], __dmul_rn((double)(idx[c] + 1), a.h[c])) - x[c]; dls[c] = (d[c] == 1.0) ? df : df / d[c]; }
+        else if (d[c] < 0.0) { const double df = __dadd_rn(a.lo[c], __dmul_rn((double)idx[c], a.h[c])) - x[c]; dls[c] = (d[c] == -1.0) ? -df : df / d[c]; }
         else dls[c] = __longlong_as_double(0x7ff0000000000000LL);
       }
       const double dl = fmax(fmin(fmin(dls[0], dls[1]), dls[2]), 0.0);        // the smallest positive solution
       const long long cell = ((long long)idx[0] * a.ny + idx[1]) * a.nz + idx[2];
       total += dl;
       // eqs. 29-31 in this cell
-      double nd[MA], add[MA];
+      double add[MA];
 #pragma unroll
-      for (int i = 0; i < MA; ++i) { nd[i] = (i < n_abs) ? a.n_dens[(long long)i * a.n_cells + cell] : 0.0; add[i] = 0.0; }
+      for (int i = 0; i < MA; ++i) add[i] = 0.0;
 #pragma unroll
       for (int b = 0; b < MB; ++b)
         if (b < n_bins) {
@@ -123,7 +136,8 @@ __global__ void __launch_bounds__(128) kr_raytrace_kernel(const KrRayArgs a) {
             if (i < n_abs) tau += nd[i] * a.sigma[i * n_bins + b] * dl;
           double e, m;
           kr_exp_pair(-tau, e, m);
-          const double f = (tau == 0.0) ? 1.0 : -m / tau;          // (1 - exp(-tau)) / tau of eqs. 28 and 30 (reading R30)
+          // (1 - exp(-tau)) / tau of eqs. 28 and 30 (reading R30); the reciprocal by krs_rcp (1 ulp, 5 instructions) for normal tau
+          const double f = (tau == 0.0) ? 1.0 : ((tau > 1e-290) ? -m * krs_rcp(tau) : -m / tau);
 #pragma unroll
           for (int i = 0; i < MA; ++i)                             // in this order: deep inside an absorber L sigma is subnormal
             if (i < n_abs) add[i] += L[b] * a.sigma[i * n_bins + b] * dl * inv_dV * f;
@@ -142,6 +156,7 @@ __global__ void __launch_bounds__(128) kr_raytrace_kernel(const KrRayArgs a) {
           x[c] = __dadd_rn(x[c], __dmul_rn(dl, d[c]));
         }
       }
+      request();
     }
   }
   if (a.L_out) {
